@@ -1,0 +1,134 @@
+/*
+ * lbm.h -- C ABI of the B200-native thermal D2Q37 Lattice-Boltzmann step (liblbm_b200.so).
+ *
+ * Implements the per-time-step update of arxiv/paper_1405_1253 (citations are PAPER.md lines):
+ * propagate (lhs of eq. 5), rigid top/bottom walls with periodic x and the
+ * BGK collision toward the force-shifted equilibrium of eq. 6 with the moments of eq. 7
+ * (PAPER.md:88), on an Lx x Lz lattice in FP64, plus the diagnostics of PAPER.md:94, 128 and eq. 12.
+ * Every arithmetic step runs in CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions.  Sites (i,k): i = 0..Lx-1 along x (periodic), k = 0..Lz-1 along z (up, walls half a site
+ * outside rows 0 and Lz-1).  Canonical dense arrays are x-fastest: fields [Lz][Lx], populations
+ * [37][Lz][Lx].  Population order: ascending e_z, then ascending e_x over all integer e with |e|^2 <= 10
+ * (l = 0 is (-1,-3), l = 18 is (0,0), l = 36 is (1,3)); the opposite of l is 36 - l.  dt = 1, c_l = r e_l,
+ * gravity (0,-g), g >= 0.  "device" pointers are CUDA device memory of the current device, "host" pointers
+ * ordinary host memory.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *
+ * Errors.  Every call returns 0 on success or a negative lbm_status; no exception crosses the boundary;
+ * lbm_last_error() returns a thread-local message for the last failing call.
+ * Ownership.  The caller owns every buffer it passes, including the two population buffers given to
+ * lbm_create (allocated e.g. by torch); the handle owns only metadata and small device scratch.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LBM_NPOP 37
+
+typedef enum {
+    LBM_OK = 0,
+    LBM_ERR_INVALID = -1, /* bad argument (size, tau, null or misaligned pointer, undersized buffer) */
+    LBM_ERR_CUDA = -2,    /* a CUDA runtime call or kernel launch failed; message has the CUDA error */
+    LBM_ERR_NODEVICE = -3 /* no CUDA device / wrong architecture */
+} lbm_status;
+
+typedef struct lbm_handle lbm_t;
+
+/* Model parameters and storage.  tau = tau_LB/dt of eq. 5 (> 1/2); g = |gravity| of eq. 3/6 (>= 0).
+ * wall_kind: 0 = half-way bounce-back through velocity-reversed mirror rows (reading 9).
+ * pop_buf0/pop_buf1: device buffers of at least lbm_buffer_bytes(Lx,Lz) bytes each, 256-byte aligned;
+ * they hold the two lattice copies (prv/nxt of PAPER.md:110) in the library's padded SoA layout. */
+typedef struct {
+    double tau;
+    double g;
+    int wall_kind;
+    void *pop_buf0; /* device */
+    void *pop_buf1; /* device */
+    size_t buf_bytes;
+} lbm_params;
+
+/* Rayleigh-Taylor initial state, eq. 1-2 with tanh-smoothed jumps.
+ * Layer temperatures T_d (bottom) > T_m > T_u (top); rho_m = density at z = 0; rho_d, rho_u follow from
+ * eq. 2.  delta = width of the middle layer in sites (0 = single front).  smooth_w = tanh
+ * half-width in sites (0 = sharp).  pert_kind: 0 none, 1 sum of n_modes cosines (amplitude uniform in
+ * [amp_lo, amp_hi], drawn only if they differ; phase uniform), 2 white noise of +-amp_hi sites per column
+ * (PAPER.md:222).  Random numbers: SplitMix64(seed), lower interface first (reading 12). */
+typedef struct {
+    double T_d, T_m, T_u;
+    double rho_m;
+    double delta;
+    double smooth_w;
+    int pert_kind;
+    int n_modes;
+    double amp_lo, amp_hi;
+} lbm_rt_init;
+
+/* Bytes each population buffer must have for an Lx x Lz lattice (padded rows, 37 planes); 0 if invalid. */
+size_t lbm_buffer_bytes(int Lx, int Lz);
+
+/* Creates a handle. Errors: Lx < 7, Lz < 6, tau <= 0.5, g < 0, wall_kind != 0, null / misaligned /
+ * undersized buffers, no sm_100 device.  *out is set to NULL on failure. */
+int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p);
+
+/* Frees the handle and its scratch; never the population buffers. NULL is a no-op. */
+int lbm_destroy(lbm_t *h);
+
+/* Fills the current lattice with the hydrostatic state of eq. 1-2 at u^(H) = 0, T^(H) = T0 (the stored
+ * populations are f_eq(rho0, (0,-g/2), T0 - g^2/8), reading 8) and resets the step counter.
+ * Synchronous with respect to the host arrays it builds; kernels run on `stream`. */
+int lbm_init_rt(lbm_t *h, uint64_t seed, const lbm_rt_init *ic, void *stream);
+
+/* Populations = f_eq(rho, u, T) of the given KINETIC fields (eq. 7; no shift). Device pointers, [Lz][Lx]. */
+int lbm_init_equilibrium(lbm_t *h, const double *rho, const double *ux, const double *uz, const double *T,
+                         void *stream);
+
+/* Canonical dense [37][Lz][Lx] populations <-> the library's layout. `f` is a DEVICE pointer
+ * (lbm_*_populations) or a HOST pointer (lbm_*_populations_host; these synchronise the stream). */
+int lbm_set_populations(lbm_t *h, const double *f_dev, void *stream);
+int lbm_get_populations(lbm_t *h, double *f_dev, void *stream);
+int lbm_set_populations_host(lbm_t *h, const double *f_host, void *stream);
+int lbm_get_populations_host(lbm_t *h, double *f_host, void *stream);
+
+/* Enqueues n x (propagate + bc + collide) on `stream`; asynchronous.  Afterwards the
+ * current lattice is the post-collision state of step n. */
+int lbm_step(lbm_t *h, int n, void *stream);
+
+/* Hydrodynamic fields of the stored state (reading 8): rho, u^(H) = u - g_vec/2,
+ * T^(H) = T + g^2/8, each a device pointer [Lz][Lx] or NULL to skip.  Asynchronous. */
+int lbm_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *stream);
+
+/* Mixing widths of eq. 12 from the x-averaged T^(H), in sites, with the
+ * tent map of eq. 9 (zero outside [0,1]).  L_u, L_d: HOST doubles; Tbar: HOST array [Lz] or NULL.
+ * Synchronises `stream`. */
+int lbm_mixing_widths(lbm_t *h, double T_d, double T_m, double T_u, double *L_u, double *L_d, double *Tbar,
+                      void *stream);
+
+/* Lattice totals sum f, sum c_x f, sum c_z f, sum |c|^2 f into HOST out[4] (deterministic two-stage
+ * reduction). Synchronises `stream`. */
+int lbm_totals(lbm_t *h, double *out4, void *stream);
+
+/* Host-buffer convenience used by the end-to-end benchmark: uploads kinetic fields (HOST, [Lz][Lx]),
+ * initialises at equilibrium, runs n steps, downloads rho, u^(H), T^(H) (HOST, [Lz][Lx], any may be NULL).
+ * Uses the handle's staging buffers (allocated on first use, 4 x Lx x Lz doubles). Synchronous. */
+int lbm_run_host(lbm_t *h, const double *rho_in, const double *ux_in, const double *uz_in, const double *T_in,
+                 int n, double *rho_out, double *ux_out, double *uz_out, double *T_out, void *stream);
+
+/* Introspection. */
+int lbm_steps_done(const lbm_t *h, long long *steps);
+int lbm_layout(const lbm_t *h, int *pitch, long long *plane_stride); /* in doubles */
+int lbm_kernel_launches(const lbm_t *h, long long *launches);       /* kernels launched through this handle */
+int lbm_set_variant(lbm_t *h, int variant);                          /* step-kernel variant */
+/* D2Q37 tables as the library uses them (host outputs, any may be NULL): e_x[37], e_z[37], w[37], r. */
+int lbm_tables(int *ex, int *ez, double *w, double *r);
+const char *lbm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */

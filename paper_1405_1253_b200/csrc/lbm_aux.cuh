@@ -1,0 +1,205 @@
+// lbm_aux.cuh -- initial states, layout conversion and the moments / diagnostics kernels (row a6).
+#pragma once
+#include <cstdint>
+
+#include "d2q37.cuh"
+#include "lbm_step.cuh"
+
+namespace lbm {
+
+struct Layout {
+    int Lx, Lz, pitch;
+    long long plane;
+};
+
+constexpr int AUX_TX = 128;  // threads per block along x for the per-site aux kernels
+constexpr int RED_T = 256;   // threads per block of the row reductions
+
+__device__ __forceinline__ void load_site(const double *src, const Layout &g, int i, int k, double (&f)[NPOP])
+{
+    const double *p = src + (long long)k * g.pitch + i;
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        f[l] = __ldg(p + (long long)l * g.plane);
+    });
+}
+
+__device__ __forceinline__ void store_site(double *dst, const Layout &g, int i, int k, const double (&f)[NPOP])
+{
+    double *p = dst + (long long)k * g.pitch + i;
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        p[(long long)l * g.plane] = f[l];
+    });
+}
+
+// populations = f_eq(rho, u, T) of given kinetic fields (dense [Lz][Lx])
+__global__ void __launch_bounds__(AUX_TX)
+init_equilibrium_kernel(double *dst, Layout g, const double *__restrict__ rho, const double *__restrict__ ux,
+                        const double *__restrict__ uz, const double *__restrict__ T)
+{
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y;
+    if (i >= g.Lx) return;
+    const long long s = (long long)k * g.Lx + i;
+    double f[NPOP];
+    d2q37::equilibrium_blend<false>(f, f, 0.0, rho[s], ux[s], uz[s], T[s]);
+    store_site(dst, g, i, k, f);
+}
+
+// Hydrostatic three-layer state, eq. 1-2 with tanh-smoothed jumps;
+// DESIGN.md reading 11.  z_k = k - (Lz-1)/2 in sites, one site = r length units, beta = 1/T0.
+struct RtArgs {
+    double g, beta_d, beta_m, beta_u, rho_m, delta, w;
+};
+
+__device__ __forceinline__ double rt_lncosh(double s)
+{
+    const double a = fabs(s);
+    return a + log1p(exp(-2.0 * a)) - 0.69314718055994530941723212145818;
+}
+__device__ __forceinline__ double rt_step(double z, double a, double w)
+{
+    if (w > 0.0) return 0.5 * (1.0 + tanh((z - a) / w));
+    return z > a ? 1.0 : (z < a ? 0.0 : 0.5);
+}
+__device__ __forceinline__ double rt_step_integral(double z, double a, double w)
+{
+    if (w > 0.0) return 0.5 * (z + w * rt_lncosh((z - a) / w) - w * rt_lncosh(a / w));
+    return fmax(z - a, 0.0) - fmax(-a, 0.0);
+}
+
+__global__ void __launch_bounds__(AUX_TX)
+init_rt_kernel(double *dst, Layout g, RtArgs p, const double *__restrict__ h_lo, const double *__restrict__ h_hi)
+{
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y;
+    if (i >= g.Lx) return;
+    const double z = (double)k - 0.5 * (double)(g.Lz - 1);
+    const double a_lo = -0.5 * p.delta + h_lo[i], a_hi = 0.5 * p.delta + h_hi[i];
+    const double dlo = p.beta_m - p.beta_d, dhi = p.beta_u - p.beta_m;
+    const double beta = p.beta_d + dlo * rt_step(z, a_lo, p.w) + dhi * rt_step(z, a_hi, p.w);
+    const double beta0 = p.beta_d + dlo * rt_step(0.0, a_lo, p.w) + dhi * rt_step(0.0, a_hi, p.w);
+    const double lnp = log(p.rho_m / beta0) -
+                       p.g * D2Q37_R *
+                           (p.beta_d * z + dlo * rt_step_integral(z, a_lo, p.w) + dhi * rt_step_integral(z, a_hi, p.w));
+    const double T0 = 1.0 / beta, rho0 = exp(lnp) * beta;
+    // stored state: u = (0, -g/2), T = T0 - g^2/8, so that u^(H) = 0 and T^(H) = T0
+    double f[NPOP];
+    d2q37::equilibrium_blend<false>(f, f, 0.0, rho0, 0.0, -0.5 * p.g, T0 - 0.125 * p.g * p.g);
+    store_site(dst, g, i, k, f);
+}
+
+// canonical dense [37][Lz][Lx]  <->  padded layout; grid = (ceil(Lx/AUX_TX), Lz, 37)
+__global__ void __launch_bounds__(AUX_TX) pack_kernel(double *dst, Layout g, const double *__restrict__ dense)
+{
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y, l = blockIdx.z;
+    if (i >= g.Lx) return;
+    dst[(long long)l * g.plane + (long long)k * g.pitch + i] = dense[((long long)l * g.Lz + k) * g.Lx + i];
+}
+__global__ void __launch_bounds__(AUX_TX) unpack_kernel(const double *__restrict__ src, Layout g, double *dense)
+{
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y, l = blockIdx.z;
+    if (i >= g.Lx) return;
+    dense[((long long)l * g.Lz + k) * g.Lx + i] = src[(long long)l * g.plane + (long long)k * g.pitch + i];
+}
+
+// Hydrodynamic fields of the stored (post-collision) state: rho, u^(H) = u - g_vec dt/2 = (u_x, u_z + g/2),
+// T^(H) = T + g^2/8 (PAPER.md:94 applied after the collision's u -> u + g_vec dt; reading 8).
+__global__ void __launch_bounds__(AUX_TX)
+moments_kernel(const double *__restrict__ src, Layout g, double grav, double *rho, double *ux, double *uz, double *T)
+{
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y;
+    if (i >= g.Lx) return;
+    double f[NPOP];
+    load_site(src, g, i, k, f);
+    const d2q37::Kinetic m = d2q37::kinetic_moments(f);
+    const long long s = (long long)k * g.Lx + i;
+    if (rho) rho[s] = m.rho;
+    if (ux) ux[s] = m.ux;
+    if (uz) uz[s] = m.uz + 0.5 * grav;
+    if (T) T[s] = m.T + 0.125 * grav * grav;
+}
+
+// deterministic block sum (fixed shuffle tree, fixed warp order); result valid in thread 0
+__device__ __forceinline__ double block_sum(double v, double *smem /* RED_T/32 doubles */)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) smem[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < RED_T / 32; ++w) t += smem[w];
+    __syncthreads();
+    return t;
+}
+
+// Tbar[k] = (1/Lx) sum_i T^(H)(i,k); one block per row
+__global__ void __launch_bounds__(RED_T) row_tbar_kernel(const double *__restrict__ src, Layout g, double grav, double *Tbar)
+{
+    __shared__ double sm[RED_T / 32];
+    const int k = blockIdx.x;
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
+        double f[NPOP];
+        load_site(src, g, i, k, f);
+        acc += d2q37::kinetic_moments(f).T + 0.125 * grav * grav;
+    }
+    const double t = block_sum(acc, sm);
+    if (threadIdx.x == 0) Tbar[k] = t / (double)g.Lx;
+}
+
+// tent map of eq. 9, zero outside (0,1)
+__device__ __forceinline__ double tent(double b)
+{
+    if (b <= 0.0 || b >= 1.0) return 0.0;
+    return b < 0.5 ? 2.0 * b : 2.0 * (1.0 - b);
+}
+
+// eq. 12: out[0] = L_u, out[1] = L_d, in sites; single block
+__global__ void __launch_bounds__(RED_T)
+widths_kernel(const double *__restrict__ Tbar, int Lz, double T_d, double T_m, double T_u, double *out)
+{
+    __shared__ double sm[RED_T / 32];
+    double lu = 0.0, ld = 0.0;
+    for (int k = threadIdx.x; k < Lz; k += RED_T) {
+        const double tb = Tbar[k];
+        lu += tent((tb - T_u) / (T_m - T_u));
+        ld += tent((tb - T_m) / (T_d - T_m));
+    }
+    const double a = block_sum(lu, sm);
+    const double b = block_sum(ld, sm);
+    if (threadIdx.x == 0) { out[0] = a; out[1] = b; }
+}
+
+// lattice totals, stage 1: per-row sums of the raw integer-velocity moments; partial[k][4]
+__global__ void __launch_bounds__(RED_T) row_totals_kernel(const double *__restrict__ src, Layout g, double *partial)
+{
+    __shared__ double sm[RED_T / 32];
+    const int k = blockIdx.x;
+    double a0 = 0, a1 = 0, a2 = 0, a3 = 0;
+    for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
+        double f[NPOP];
+        load_site(src, g, i, k, f);
+        const d2q37::RawMoments m = d2q37::raw_moments(f);
+        a0 += m.m0; a1 += m.jx; a2 += m.jz; a3 += m.m2;
+    }
+    const double s0 = block_sum(a0, sm), s1 = block_sum(a1, sm), s2 = block_sum(a2, sm), s3 = block_sum(a3, sm);
+    if (threadIdx.x == 0) {
+        partial[4 * k + 0] = s0; partial[4 * k + 1] = s1; partial[4 * k + 2] = s2; partial[4 * k + 3] = s3;
+    }
+}
+
+// stage 2: out = (sum f, sum c_x f, sum c_z f, sum |c|^2 f), c = r e; single block
+__global__ void __launch_bounds__(RED_T) final_totals_kernel(const double *__restrict__ partial, int Lz, double *out)
+{
+    __shared__ double sm[RED_T / 32];
+    double a[4] = {0, 0, 0, 0};
+    for (int k = threadIdx.x; k < Lz; k += RED_T)
+        for (int j = 0; j < 4; ++j) a[j] += partial[4 * k + j];
+    const double s0 = block_sum(a[0], sm), s1 = block_sum(a[1], sm), s2 = block_sum(a[2], sm), s3 = block_sum(a[3], sm);
+    if (threadIdx.x == 0) {
+        out[0] = s0; out[1] = D2Q37_R * s1; out[2] = D2Q37_R * s2; out[3] = D2Q37_R2 * s3;
+    }
+}
+
+}  // namespace lbm

@@ -1,0 +1,103 @@
+// lbm_step.cuh -- the fused propagate + bc + collide kernel (one launch per time step).
+//
+// Store: structure of arrays, f[l][k][i] at  l*plane + k*pitch + i  doubles,
+// x fastest, rows padded to a multiple of 16 doubles (128 B), two copies (src = prv, dst = nxt of
+// PAPER.md:110).  One thread updates one site:
+//   a1/a2  pull-propagate with periodic x: 37 gathers from src at (i - e_x mod Lx, k - e_z)
+//   a3     walls: a source row below 0 / above Lz-1 is replaced by the mirror row and the opposite
+//          population (pure index remap, block-uniform because a block works on one row)
+//   a4     collide in registers (d2q37.cuh), 37 aligned stores to dst
+// No halo rows or wrap columns are stored: the wrap is seven per-thread column indices, the walls are
+// seven block-uniform (row, flip) pairs, so interior blocks run a branch-free path.
+#pragma once
+#include <cstdint>
+
+#include "d2q37.cuh"
+
+namespace lbm {
+
+using d2q37::NPOP;
+
+struct StepArgs {
+    const double *src;
+    double *dst;
+    int Lx, Lz;
+    int pitch;          // doubles per row
+    long long plane;    // doubles per population plane
+    double omega;       // dt / tau
+    double gtau;        // g tau
+    double dT;          // tau (1 - tau) g^2 / 2
+};
+
+// streaming load / store: every population value is read once and written once per step
+__device__ __forceinline__ double ld_stream(const double *p)
+{
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_stream(double *p, double v)
+{
+    asm volatile("st.global.L1::no_allocate.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
+// Gather the 37 post-propagate populations of site (i, k).  WALL = false: rows 3..Lz-4, no remap.
+template <bool WALL>
+__device__ __forceinline__ void gather_site(const StepArgs &a, int i, int k, double (&f)[NPOP])
+{
+    // periodic x (a1): wrapped source column for each e_x in -3..3
+    int col[7];
+#pragma unroll
+    for (int d = -3; d <= 3; ++d) {
+        int c = i - d;
+        c += (c < 0) ? a.Lx : 0;
+        c -= (c >= a.Lx) ? a.Lx : 0;
+        col[d + 3] = c;
+    }
+    // source row for each e_z in -3..3, with the wall remap (a3)
+    long long rowoff[7];
+    bool flip[7];
+#pragma unroll
+    for (int d = -3; d <= 3; ++d) {
+        int ks = k - d;
+        bool fl = false;
+        if (WALL) {
+            if (ks < 0) { ks = -1 - ks; fl = true; }
+            else if (ks >= a.Lz) { ks = 2 * a.Lz - 1 - ks; fl = true; }
+        }
+        rowoff[d + 3] = (long long)ks * a.pitch;
+        flip[d + 3] = fl;
+    }
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        constexpr int ex = d2q37::pop_ex(l), ez = d2q37::pop_ez(l);
+        int ls = l;
+        if (WALL) ls = flip[ez + 3] ? (NPOP - 1 - l) : l;
+        f[l] = ld_stream(a.src + (long long)ls * a.plane + rowoff[ez + 3] + col[ex + 3]);
+    });
+}
+
+__device__ __forceinline__ void scatter_site(const StepArgs &a, int i, int k, const double (&f)[NPOP])
+{
+    double *p = a.dst + (long long)k * a.pitch + i;
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        st_stream(p + (long long)l * a.plane, f[l]);
+    });
+}
+
+// v0: one thread per site, block = TX consecutive columns of one row, grid = (ceil(Lx/TX), Lz).
+template <int TX>
+__global__ void __launch_bounds__(TX) step_kernel_site(const StepArgs a)
+{
+    const int i = blockIdx.x * TX + threadIdx.x;
+    const int k = blockIdx.y;
+    if (i >= a.Lx) return;
+    double f[NPOP];
+    if (k >= 3 && k < a.Lz - 3) gather_site<false>(a, i, k, f);
+    else gather_site<true>(a, i, k, f);
+    d2q37::collide_site(f, a.omega, a.gtau, a.dT);
+    scatter_site(a, i, k, f);
+}
+
+}  // namespace lbm

@@ -1,0 +1,95 @@
+"""CPU tier for the CUDA library: it builds, exports every symbol of include/lbm.h, its host-side logic
+(argument checks, buffer sizes, tables) behaves, and the product path has no CPU fallback.
+No compute call is made here (there is no GPU)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import __graft_entry__ as g
+    g.build()
+    from paper_1405_1253_b200 import binding
+    return binding.load()
+
+
+def test_library_exports_every_declared_symbol(lib):
+    from paper_1405_1253_b200 import binding
+    header = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    declared = set(re.findall(r"\b(lbm_[a-z_]+)\s*\(", header))
+    assert declared == set(binding.SYMBOLS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_buffer_bytes_and_layout_rules(lib):
+    assert lib.lbm_buffer_bytes(6, 128) == 0 and lib.lbm_buffer_bytes(64, 5) == 0
+    for Lx, Lz in [(64, 128), (100, 37), (4096, 8192)]:
+        b = lib.lbm_buffer_bytes(Lx, Lz)
+        pitch = (Lx + 15) // 16 * 16
+        assert b >= 37 * pitch * Lz * 8 and b % 128 == 0
+        plane = b // 37
+        assert plane % 128 == 0                       # plane bases stay on 128-byte lines
+        assert (plane // 128) % 2 == 1 or Lx % 32     # ... and off power-of-two strides
+
+
+def test_tables_match_paper_constants(lib):
+    """The library's own tables satisfy the same paper pins as the oracle's (M = 37, r ~ 1.1969,
+    PAPER.md:75, 100) and the Gaussian moment conditions -- checked independently of the oracle."""
+    import paper_1405_1253_b200 as pkg
+    ex, ez, w, r = pkg.tables()
+    ex, ez, w = np.array(ex), np.array(ez), np.array(w)
+    assert len(ex) == 37 and int(r * 1e4) == 11969
+    assert np.all(ex[::-1] == -ex) and np.all(ez[::-1] == -ez) and abs(w.sum() - 1) < 1e-15
+    for a, b, want in [(2, 0, 1), (4, 0, 3), (2, 2, 1), (6, 0, 15), (4, 2, 3), (8, 0, 105), (6, 2, 15), (4, 4, 9)]:
+        assert abs(np.sum(w * (r * ex) ** a * (r * ez) ** b) - want) < 1e-12 * want
+
+
+def test_create_rejects_bad_arguments_before_touching_a_device(lib):
+    from paper_1405_1253_b200.binding import lbm_params
+    h = C.c_void_p()
+    good = dict(tau=0.8, g=1e-4, wall_kind=0, pop_buf0=256, pop_buf1=512, buf_bytes=1 << 40)
+    for bad in [dict(tau=0.5), dict(g=-1.0), dict(wall_kind=3), dict(pop_buf0=0), dict(pop_buf1=256),
+                dict(pop_buf0=264), dict(buf_bytes=16)]:
+        p = lbm_params(**{**good, **bad})
+        assert lib.lbm_create(C.byref(h), 64, 128, C.byref(p)) == -1, bad
+        assert h.value is None and lib.lbm_last_error()
+    p = lbm_params(**good)
+    assert lib.lbm_create(C.byref(h), 3, 128, C.byref(p)) == -1
+    assert lib.lbm_create(C.byref(h), 64, 128, None) == -1
+    assert lib.lbm_step(None, 1, None) == -1 and lib.lbm_destroy(None) == 0
+
+
+def test_no_cpu_fallback_and_no_oracle_on_the_product_path():
+    """The package never imports oracle/ and refuses to run without a device."""
+    import torch
+    import paper_1405_1253_b200 as pkg
+    pkgdir = os.path.dirname(pkg.__file__)
+    for dirpath, _, files in os.walk(pkgdir):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "lbm_oracle" not in src, fn
+    if not torch.cuda.is_available():
+        with pytest.raises(pkg.LbmError):
+            pkg.Lattice(64, 128, 0.8, 1e-4)
+
+
+def test_synthetic_inputs_are_reproducible_and_sliceable():
+    import synthetic_inputs as si
+    full = si.sweep_fields(32, 24, seed=5)
+    part = si.sweep_fields(32, 24, seed=5, rows=slice(7, 12))
+    for a, b in zip(full, part):
+        assert np.array_equal(a[7:12], b)
+    rho, ux, uz, T = full
+    assert abs(rho.mean() - 1) < 2e-3 and np.all(np.abs(rho - 1) <= 0.01) and np.all(np.abs(ux) <= 0.01)
+    assert np.all(np.abs(T - 1) <= 0.01) and np.all(np.abs(uz) <= 0.01)
+    cfg = si.rt_config(4)
+    assert (cfg.Lx, cfg.Lz, cfg.delta, cfg.pert_kind) == (4096, 8192, 0.0, si.PERT_WHITE)
+    assert si.scaled(si.rt_config(2), 128, 256).delta == 64
