@@ -1,0 +1,160 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (north_star): max relative error per population <= 1e-11 after 100 steps,
+conserved totals to 1e-12 relative.  Run on the B200 box: pytest -m gpu."""
+import numpy as np
+import pytest
+
+import synthetic_inputs as si
+
+pytestmark = pytest.mark.gpu
+
+POP_RTOL = 1e-11
+TOT_RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import __graft_entry__ as g
+    g.build()
+    import paper_1405_1253_b200 as p
+    return p
+
+
+def _rel(a, b):
+    return float(np.max(np.abs(a - b) / np.abs(b)))
+
+
+def _oracle_rt(orc, cfg, seed, nsteps):
+    f0 = orc.init_rt(cfg.Lx, cfg.Lz, cfg.g, seed, **cfg.rt_args())
+    return f0, orc.step(f0, cfg.tau, cfg.g, nsteps=nsteps)
+
+
+def test_tables_agree_with_oracle(pkg, orc):
+    ex, ez, w, r = pkg.tables()
+    oex, oez, ow, orr = orc.tables()
+    assert list(oex) == ex and list(oez) == ez
+    assert np.max(np.abs(np.array(w) / ow - 1)) < 4e-16 and abs(r / orr - 1) < 4e-16
+
+
+def test_config1_init_matches_oracle(pkg, orc):
+    cfg = si.rt_config(1)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    got = lat.get_populations(host=True).numpy()
+    ref = orc.init_rt(cfg.Lx, cfg.Lz, cfg.g, si.DEFAULT_SEED, **cfg.rt_args())
+    assert _rel(got, ref) < 1e-13        # exp/tanh/log1p differ by an ulp or two between libm and CUDA
+    lat.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config1_100_steps_population_parity(pkg, orc, variant):
+    """BASELINE.json configs[0]: 64x128 double-front RT, 100 steps, every population of every site."""
+    cfg = si.rt_config(1)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    lat.set_variant(variant)
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    lat.step(cfg.steps)
+    assert lat.steps_done == 100
+    got = lat.get_populations(host=True).numpy()
+    _, ref = _oracle_rt(orc, cfg, si.DEFAULT_SEED, cfg.steps)
+    assert _rel(got, ref) < POP_RTOL
+    tg, tr = lat.totals(), orc.totals(ref)
+    assert abs(tg[0] / tr[0] - 1) < TOT_RTOL and abs(tg[3] / tr[3] - 1) < TOT_RTOL
+    assert abs(tg[1] - tr[1]) < TOT_RTOL * tr[0] and abs(tg[2] - tr[2]) < TOT_RTOL * tr[0]
+    lat.close()
+
+
+@pytest.mark.parametrize("Lx,Lz,steps", [(7, 6, 5), (33, 9, 12), (130, 70, 20), (257, 40, 10), (520, 18, 7)])
+def test_ragged_and_tiny_lattices_from_identical_populations(pkg, orc, Lx, Lz, steps):
+    """Same starting populations on both sides (uploaded), odd sizes: minimum lattice, ragged block tails,
+    lattices where every row is a wall row, several blocks per row."""
+    rng = np.random.default_rng(Lx * 1000 + Lz)
+    rho = 1 + 0.05 * rng.uniform(-1, 1, (Lz, Lx)); T = 1 + 0.05 * rng.uniform(-1, 1, (Lz, Lx))
+    ux = 0.03 * rng.uniform(-1, 1, (Lz, Lx)); uz = 0.03 * rng.uniform(-1, 1, (Lz, Lx))
+    f0 = orc.init_equilibrium(rho, ux, uz, T) * (1 + 0.01 * rng.uniform(-1, 1, (37, Lz, Lx)))
+    import torch
+    lat = pkg.Lattice(Lx, Lz, 0.63, 2e-4)
+    lat.set_populations(torch.from_numpy(f0))                 # host path
+    assert np.array_equal(lat.get_populations(host=True).numpy(), f0)   # layout round trip is bit exact
+    lat.step(steps)
+    got = lat.get_populations().cpu().numpy()                 # device path
+    ref = orc.step(f0, 0.63, 2e-4, nsteps=steps)
+    assert _rel(got, ref) < POP_RTOL
+    lat.close()
+
+
+def test_single_step_walls_and_wrap_exact_structure(pkg, orc):
+    """One step from a state where every (l, i, k) value is distinct: any wrong source index (wrap,
+    wall mirror, opposite population) changes the result at O(1), far above rounding."""
+    Lx, Lz = 19, 11
+    l, k, i = np.meshgrid(np.arange(37), np.arange(Lz), np.arange(Lx), indexing="ij")
+    f0 = orc.feq(1.0, 0.0, 0.0, 1.0)[:, None, None] * (1 + 0.3 * np.sin(1.0 + 0.7 * l + 1.3 * k + 2.1 * i))
+    import torch
+    lat = pkg.Lattice(Lx, Lz, 0.9, 1e-3)
+    lat.set_populations(torch.from_numpy(f0).cuda())
+    lat.step(1)
+    got = lat.get_populations(host=True).numpy()
+    assert _rel(got, orc.step(f0, 0.9, 1e-3, nsteps=1)) < 1e-13
+    lat.close()
+
+
+def test_init_equilibrium_moments_and_widths(pkg, orc):
+    import torch
+    Lx, Lz, g = 96, 80, 1e-4
+    rho, ux, uz, T = si.sweep_fields(Lx, Lz, seed=3)
+    z = np.arange(Lz)[:, None]
+    T = T + 0.05 * np.tanh((z - 40) / 6.0) * -1.0            # a front so that the widths are not trivial
+    lat = pkg.Lattice(Lx, Lz, 0.8, g)
+    lat.init_equilibrium(*[torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (rho, ux, uz, T)])
+    f0 = orc.init_equilibrium(rho, ux, uz, T)
+    assert _rel(lat.get_populations(host=True).numpy(), f0) < 1e-13
+    lat.step(3)
+    ref = orc.step(f0, 0.8, g, nsteps=3)
+    m = [x.cpu().numpy() for x in lat.moments()]
+    mo = orc.moments(ref, g)
+    assert np.max(np.abs(m[0] - mo[0])) < 1e-13 and np.max(np.abs(m[3] - mo[3])) < 1e-13
+    assert np.max(np.abs(m[1] - mo[1])) < 1e-14 and np.max(np.abs(m[2] - mo[2])) < 1e-14
+    lu, ld, tbar = lat.mixing_widths(1.05, 1.0, 0.95)
+    olu, old, otbar = orc.mixing_widths(ref, g, 1.05, 1.0, 0.95)
+    assert np.max(np.abs(tbar - otbar)) < 1e-13 and abs(lu - olu) < 1e-10 and abs(ld - old) < 1e-10
+    assert lu > 1 and ld > 1
+    # only-T request leaves the other outputs untouched (null pointers are skipped)
+    Tonly = torch.empty((Lz, Lx), dtype=torch.float64, device="cuda")
+    lat.moments(T=Tonly, alloc=False)
+    assert np.array_equal(Tonly.cpu().numpy(), m[3])
+    lat.close()
+
+
+def test_conservation_and_invariants_on_gpu(pkg):
+    """Properties that hold at any size, on the CUDA path alone: mass and (without gravity) energy are
+    conserved by walls + collision to rounding -- momentum is not, rigid walls absorb it -- and
+    x-translation invariance is bit exact."""
+    import torch
+    Lx, Lz = 160, 96
+    rho, ux, uz, T = [torch.from_numpy(x).cuda() for x in si.sweep_fields(Lx, Lz, seed=11)]
+    lat = pkg.Lattice(Lx, Lz, 0.7, 0.0)
+    lat.init_equilibrium(rho, ux, uz, T)
+    t0 = lat.totals(); lat.step(50); t1 = lat.totals()
+    assert abs(t1[0] / t0[0] - 1) < 1e-13 and abs(t1[3] / t0[3] - 1) < 1e-13
+    a = lat.get_populations()
+    lat2 = pkg.Lattice(Lx, Lz, 0.7, 0.0)
+    lat2.init_equilibrium(*[torch.roll(x, 37, dims=1).contiguous() for x in (rho, ux, uz, T)])
+    lat2.step(50)
+    assert torch.equal(torch.roll(a, 37, dims=2), lat2.get_populations())
+    lat.close(); lat2.close()
+
+
+def test_run_host_end_to_end(pkg, orc):
+    import torch
+    Lx, Lz, g = 64, 48, 1e-4
+    fields = si.sweep_fields(Lx, Lz, seed=2)
+    lat = pkg.Lattice(Lx, Lz, 0.8, g)
+    ins = [torch.from_numpy(x).pin_memory() for x in fields]
+    outs = lat.run_host(*ins, n=4)
+    ref = orc.moments(orc.step(orc.init_equilibrium(*fields), 0.8, g, nsteps=4), g)
+    for o, r_ in zip(outs, ref):
+        assert np.max(np.abs(o.numpy() - r_)) < 1e-13
+    lat.close()
