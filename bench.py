@@ -47,7 +47,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, device_index: int):
         super().__init__(daemon=True)
         self.samples, self.mask, self.max_mhz, self.ok = [], 0, None, False
-        self._stop = threading.Event()
+        self._halt = threading.Event()
         try:
             import pynvml
             import torch
@@ -64,7 +64,7 @@ class ClockSampler(threading.Thread):
             self.err = repr(e)
 
     def run(self):
-        while self.ok and not self._stop.is_set():
+        while self.ok and not self._halt.is_set():
             try:
                 self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
                 self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
@@ -73,7 +73,7 @@ class ClockSampler(threading.Thread):
             time.sleep(0.02)
 
     def finish(self) -> dict:
-        self._stop.set()
+        self._halt.set()
         if self.is_alive():
             self.join()
         if not self.samples:
@@ -130,3 +130,142 @@ def run_reference(args):
         "e2e": {"value": mlups, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import __graft_entry__ as entry
+    import paper_1405_1253_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        entry.build()
+    if world > 1:
+        dist.barrier()
+
+    cfg = si.rt_config(args.config)
+    if args.lx and args.lz:
+        cfg = si.scaled(cfg, args.lx, args.lz)
+    sites = cfg.Lx * cfg.Lz
+    stream = torch.cuda.current_stream()
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    if args.variant is not None:
+        lat.set_variant(args.variant)
+    lat.init_rt(si.DEFAULT_SEED + rank, **cfg.rt_args())     # replicas differ only by their seed
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps + one widths call
+    lat.step(args.warmup)
+    lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = lat.kernel_launches
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ev[0].record(stream)
+    lat.step(args.steps)                                     # K launches of the fused step kernel
+    ev[1].record(stream)
+    widths = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)   # a6, synchronises
+    ev[2].record(stream)
+    barrier()
+    clocks = sampler.finish()
+    launches = lat.kernel_launches - l0
+    t_steps = ev[0].elapsed_time(ev[1]) * 1e-3
+    t_total = ev[0].elapsed_time(ev[2]) * 1e-3
+    times = torch.tensor([t_total, t_steps], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    t_total, t_steps = (float(x) for x in times.cpu())
+    value = world * sites * args.steps / t_total / 1e6
+
+    # ---- end to end through lbm_run_host: pinned host fields in, K steps, host fields out
+    g = cfg.g
+    rho, ux, uz, T = lat.moments()
+    host_in = [x.cpu().pin_memory() for x in (rho, ux, uz - 0.5 * g, T - 0.125 * g * g)]  # kinetic fields
+    host_out = tuple(torch.empty_like(x).pin_memory() for x in host_in)
+    del rho, ux, uz, T
+    e2e_steps = args.e2e_steps or args.steps
+    lat.run_host(*host_in, n=min(3, e2e_steps), outs=host_out)          # warm-up (allocates staging)
+    barrier()
+    t0 = time.perf_counter()
+    lat.run_host(*host_in, n=e2e_steps, outs=host_out)                   # synchronous
+    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+    t_e2e = float(t_e2e.cpu())
+    field_bytes = 4 * 8 * sites
+    e2e = {"value": world * sites * e2e_steps / t_e2e / 1e6, "unit": "MLUPS", "steps": e2e_steps,
+           "h2d_bytes_per_step": field_bytes / e2e_steps, "d2h_bytes_per_step": field_bytes / e2e_steps,
+           "call": "lbm_run_host (pinned host rho,u,T in -> init -> K steps -> host rho,u,T out)"}
+    lat.close()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_kind = measured_peak()
+    step_ms = t_steps / args.steps * 1e3
+    achieved = BYTES_PER_SITE * sites / (t_steps / args.steps) / 1e9
+    roofline = {"bound": "hbm", "kernel": "step_kernel (fused propagate+bc+collide)", "achieved": achieved,
+                "peak": peak, "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
+                "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
+                "bytes_per_site": BYTES_PER_SITE, "kernel_ms": step_ms, "traffic": NCU_TRAFFIC_BYTES}
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, cores, sample = oracle_sample_rate(cfg, args.cpu_budget)
+        cpu = {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample}
+    print(json.dumps({
+        "metric": "MLUPS (FP64)", "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t_total / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "Lx": cfg.Lx, "Lz": cfg.Lz, "tau": cfg.tau, "g": cfg.g,
+                   "parallelism": "replicas only" if world > 1 else "single GPU, whole lattice resident",
+                   "l2": "inputs larger than L2 (2 x 37 planes, %.1f GB)" % (2 * 37 * 8 * sites / 1e9),
+                   "variant": args.variant, "widths_calls_in_timed_region": 1,
+                   "L_u": widths[0], "L_d": widths[1]},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+    }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="RT config 1..4 of BASELINE.json (default 4: 4096x8192)")
+    ap.add_argument("--lx", type=int, default=0)
+    ap.add_argument("--lz", type=int, default=0)
+    ap.add_argument("--variant", type=int, default=None, help="step-kernel variant (default: library default)")
+    ap.add_argument("--e2e-steps", type=int, default=0)
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle time for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
