@@ -27,8 +27,8 @@ import synthetic_inputs as si  # noqa: E402
 BYTES_PER_SITE = 592          # 37 x 8 B read + 37 x 8 B written per site per step
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel at 4096x8192, from the committed
-# `ncu --set full` capture (profiles/); None until a capture exists for the default variant.
-NCU_TRAFFIC_BYTES = None
+# `ncu --set full` capture (profiles/), keyed by (workload, variant); null for anything not captured.
+NCU_TRAFFIC_BYTES = {("rt_single_4096x8192", 0): 19.814e9}   # profiles/r1_step_kernel_full.md
 
 
 def measured_peak():
@@ -133,6 +133,21 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------ our arm
+def reduce_max(values, world: int, device: str):
+    """MAX over ranks of a list of per-rank timings (one process per GPU; gloo on CPU in the tests)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def whole_job_mlups(sites_per_rank: int, steps: int, world: int, seconds_max: float) -> float:
+    """Replicas only: every rank updates its own lattice; the job's rate is all sites over the slowest rank."""
+    return world * sites_per_rank * steps / seconds_max / 1e6
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -187,11 +202,8 @@ def run_ours(args):
     launches = lat.kernel_launches - l0
     t_steps = ev[0].elapsed_time(ev[1]) * 1e-3
     t_total = ev[0].elapsed_time(ev[2]) * 1e-3
-    times = torch.tensor([t_total, t_steps], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    t_total, t_steps = (float(x) for x in times.cpu())
-    value = world * sites * args.steps / t_total / 1e6
+    t_total, t_steps = reduce_max([t_total, t_steps], world, "cuda")
+    value = whole_job_mlups(sites, args.steps, world, t_total)
 
     # ---- end to end through lbm_run_host: pinned host fields in, K steps, host fields out
     g = cfg.g
@@ -204,12 +216,9 @@ def run_ours(args):
     barrier()
     t0 = time.perf_counter()
     lat.run_host(*host_in, n=e2e_steps, outs=host_out)                   # synchronous
-    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-    t_e2e = float(t_e2e.cpu())
+    t_e2e = reduce_max([time.perf_counter() - t0], world, "cuda")[0]
     field_bytes = 4 * 8 * sites
-    e2e = {"value": world * sites * e2e_steps / t_e2e / 1e6, "unit": "MLUPS", "steps": e2e_steps,
+    e2e = {"value": whole_job_mlups(sites, e2e_steps, world, t_e2e), "unit": "MLUPS", "steps": e2e_steps,
            "h2d_bytes_per_step": field_bytes / e2e_steps, "d2h_bytes_per_step": field_bytes / e2e_steps,
            "call": "lbm_run_host (pinned host rho,u,T in -> init -> K steps -> host rho,u,T out)"}
     lat.close()
@@ -225,7 +234,7 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": "step_kernel (fused propagate+bc+collide)", "achieved": achieved,
                 "peak": peak, "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
                 "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
-                "bytes_per_site": BYTES_PER_SITE, "kernel_ms": step_ms, "traffic": NCU_TRAFFIC_BYTES}
+                "bytes_per_site": BYTES_PER_SITE, "kernel_ms": step_ms, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, args.variant or 0))}
     cpu = None
     if not args.no_cpu_baseline:
         v, cores, sample = oracle_sample_rate(cfg, args.cpu_budget)
