@@ -254,6 +254,47 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """--sweep: BASELINE.json configs[4] -- steady-state throughput from 256x512 to 8192x16384, populations at
+    the equilibrium of i.i.d. rho, T, u fields; 200 timed steps per size (after 10 warm-up), one JSON line per
+    (size, variant) with MLUPS, algorithmic GB/s and the moments kernel's rate.  Not the driver's contract line."""
+    import torch
+
+    import __graft_entry__ as entry
+    import paper_1405_1253_b200 as pkg
+    entry.build()
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    peak, _ = measured_peak()
+    variants = [int(v) for v in args.sweep_variants.split(",")]
+    sizes = [tuple(int(x) for x in sz.split("x")) for sz in args.sweep_sizes.split(",")] if args.sweep_sizes \
+        else si.SWEEP_SIZES
+    for Lx, Lz in sizes:
+        sites = Lx * Lz
+        fields = si.sweep_fields_torch(Lx, Lz, si.DEFAULT_SEED, "cuda")
+        lat = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G)
+        for v in variants:
+            lat.set_variant(v)
+            lat.init_equilibrium(*fields)
+            lat.step(args.warmup)
+            torch.cuda.synchronize()
+            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            e0.record(stream); lat.step(args.steps); e1.record(stream)
+            lat.moments(*fields); e2.record(stream)            # overwrites the input fields: re-drawn per size
+            torch.cuda.synchronize()
+            t = e0.elapsed_time(e1) * 1e-3 / args.steps
+            tm = e1.elapsed_time(e2) * 1e-3
+            tot = lat.totals()
+            print(json.dumps({"sweep": f"{Lx}x{Lz}", "variant": v, "mlups": sites / t / 1e6, "us_per_step": t * 1e6,
+                              "gbs": BYTES_PER_SITE * sites / t / 1e9, "frac_of_measured_peak": BYTES_PER_SITE * sites / t / 1e9 / peak,
+                              "resident": "L2" if 2 * 37 * 8 * sites < 126e6 else "HBM",
+                              "moments_gbs": 328 * sites / tm / 1e9, "mass": tot[0]}), flush=True)
+            fields = si.sweep_fields_torch(Lx, Lz, si.DEFAULT_SEED, "cuda")
+        lat.close()
+        del fields, lat
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -267,10 +308,15 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=0)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="config 5: throughput sweep over lattice sizes")
+    ap.add_argument("--sweep-variants", default="0")
+    ap.add_argument("--sweep-sizes", default="", help="e.g. 256x512,4096x8192 (default: all of config 5)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -256,12 +256,12 @@ int lbm_step(lbm_t *h, int n, void *stream)
         a.src = h->buf[h->cur];
         a.dst = h->buf[h->cur ^ 1];
         switch (h->variant) {
-        case 1:
-            lbm::step_kernel_site<128><<<site_grid(h, 128), 128, 0, st>>>(a);
-            break;
-        default:  // 256 threads = 2 blocks/SM at 128 registers: measured fastest at 4096x8192
-            lbm::step_kernel_site<256><<<site_grid(h, 256), 256, 0, st>>>(a);
-            break;
+#define LBM_LAUNCH_SITE(TX, TZ)                                                                          \
+    lbm::step_kernel_site<TX, TZ><<<dim3((h->Lx + TX - 1) / TX, (h->Lz + TZ - 1) / TZ), dim3(TX, TZ), 0, st>>>(a)
+        case 1: LBM_LAUNCH_SITE(128, 1); break;
+        case 2: LBM_LAUNCH_SITE(128, 2); break;
+        default: LBM_LAUNCH_SITE(256, 1); break;  // 2 blocks/SM at 128 registers: measured fastest at 4096x8192
+#undef LBM_LAUNCH_SITE
         }
         LAUNCHED(h);
         h->cur ^= 1;  // a5: swap prv / nxt
@@ -362,7 +362,7 @@ int lbm_kernel_launches(const lbm_t *h, long long *launches)
 int lbm_set_variant(lbm_t *h, int variant)
 {
     NEED(h);
-    if (variant < 0 || variant > 1) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
+    if (variant < 0 || variant > 2) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
     h->variant = variant;
     return LBM_OK;
 }

@@ -86,13 +86,14 @@ __device__ __forceinline__ void scatter_site(const StepArgs &a, int i, int k, co
     });
 }
 
-// v0: one thread per site, block = TX consecutive columns of one row, grid = (ceil(Lx/TX), Lz).
-template <int TX>
-__global__ void __launch_bounds__(TX) step_kernel_site(const StepArgs a)
+// One thread per site; a block covers TX consecutive columns of TZ consecutive rows,
+// grid = (ceil(Lx/TX), ceil(Lz/TZ)).  The wall test is per row, hence warp-uniform (TX is a multiple of 32).
+template <int TX, int TZ>
+__global__ void __launch_bounds__(TX *TZ) step_kernel_site(const StepArgs a)
 {
     const int i = blockIdx.x * TX + threadIdx.x;
-    const int k = blockIdx.y;
-    if (i >= a.Lx) return;
+    const int k = blockIdx.y * TZ + threadIdx.y;
+    if (i >= a.Lx || k >= a.Lz) return;
     double f[NPOP];
     if (k >= 3 && k < a.Lz - 3) gather_site<false>(a, i, k, f);
     else gather_site<true>(a, i, k, f);

@@ -112,3 +112,36 @@ def sweep_fields(Lx: int, Lz: int, seed: int = DEFAULT_SEED, rows: slice | None 
     uz = 0.01 * (2.0 * u[..., 3] - 1.0)
     return (np.ascontiguousarray(rho), np.ascontiguousarray(ux), np.ascontiguousarray(uz),
             np.ascontiguousarray(T))
+
+
+def _splitmix64_uniform_torch(seed: int, first: int, count: int, device):
+    """Same stream as splitmix64_uniform, evaluated with torch int64 arithmetic (wraps mod 2^64) on `device`."""
+    import torch
+
+    def s64(v):  # two's-complement view of a uint64 constant
+        v &= 0xFFFFFFFFFFFFFFFF
+        return v - (1 << 64) if v >= (1 << 63) else v
+
+    def lsr(z, n):  # logical shift right on int64
+        return (z >> n) & ((1 << (64 - n)) - 1)
+
+    n = torch.arange(first + 1, first + count + 1, dtype=torch.int64, device=device)
+    z = n * s64(0x9E3779B97F4A7C15) + s64(seed)
+    z = (z ^ lsr(z, 30)) * s64(0xBF58476D1CE4E5B9)
+    z = (z ^ lsr(z, 27)) * s64(0x94D049BB133111EB)
+    z = z ^ lsr(z, 31)
+    return lsr(z, 11).to(torch.float64) * (1.0 / 9007199254740992.0)
+
+
+def sweep_fields_torch(Lx: int, Lz: int, seed: int = DEFAULT_SEED, device="cuda", chunk_rows: int = 1024):
+    """sweep_fields() produced directly on `device` (bit-identical values), in row chunks to bound memory."""
+    import torch
+    out = [torch.empty((Lz, Lx), dtype=torch.float64, device=device) for _ in range(4)]
+    for k0 in range(0, Lz, chunk_rows):
+        k1 = min(Lz, k0 + chunk_rows)
+        u = _splitmix64_uniform_torch(seed, 4 * k0 * Lx, 4 * (k1 - k0) * Lx, device).reshape(k1 - k0, Lx, 4)
+        out[0][k0:k1] = 1.0 + 0.01 * (2.0 * u[..., 0] - 1.0)      # rho
+        out[3][k0:k1] = 1.0 + 0.01 * (2.0 * u[..., 1] - 1.0)      # T
+        out[1][k0:k1] = 0.01 * (2.0 * u[..., 2] - 1.0)            # u_x
+        out[2][k0:k1] = 0.01 * (2.0 * u[..., 3] - 1.0)            # u_z
+    return tuple(out)

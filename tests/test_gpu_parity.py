@@ -49,7 +49,7 @@ def test_config1_init_matches_oracle(pkg, orc):
     lat.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_config1_100_steps_population_parity(pkg, orc, variant):
     """BASELINE.json configs[0]: 64x128 double-front RT, 100 steps, every population of every site."""
     cfg = si.rt_config(1)
