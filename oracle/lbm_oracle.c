@@ -521,3 +521,62 @@ void orc_init_rt(double *f, int Lx, int Lz, double g, uint64_t seed, double T_d,
     if (T0_out) memcpy(T0_out, T0, sizeof(double) * plane);
     free(h_lo); free(h_hi); free(rho0); free(T0);
 }
+
+/* ---------------------------------------------------------------------------------------
+ * Row profiles used in section IV of the paper, from the hydrodynamic fields of the stored
+ * state:
+ *   Tbar(k)  = <T>_x
+ *   Trms(k)  = sqrt( < (T - <T>_x)^2 >_x )             (Fig. 8)
+ *   Ekbar(k) = <E_k>_x,  Ekrms(k) = sqrt( < (E_k - <E_k>_x)^2 >_x )   (Fig. 9)
+ * READING (the paper does not define E_k): E_k = rho |u^(H)|^2 / 2, the kinetic energy
+ * density.  Two passes per row (mean, then squared deviations).  Pinned by closed forms on
+ * cosine-modulated rows; parity with the authors' E_k definition is UNPINNED.
+ * Any output (length Lz) may be NULL.
+ * ------------------------------------------------------------------------------------- */
+void orc_profiles(const double *f, int Lx, int Lz, double g, double *Tbar, double *Trms, double *Ekbar,
+                  double *Ekrms)
+{
+    ensure_tables();
+    const size_t plane = (size_t)Lx * (size_t)Lz;
+    double *Trow = (double *)malloc(sizeof(double) * Lx), *Erow = (double *)malloc(sizeof(double) * Lx);
+    for (int k = 0; k < Lz; ++k) {
+        double sT = 0.0, sE = 0.0;
+        for (int i = 0; i < Lx; ++i) {
+            const size_t s = (size_t)k * Lx + i;
+            double fl[NPOP], m0, vx, vz, t;
+            for (int l = 0; l < NPOP; ++l) fl[l] = f[l * plane + s];
+            site_moments(fl, &m0, &vx, &vz, &t);
+            const double uzh = vz + 0.5 * g;
+            Trow[i] = t + g * g / (4.0 * DIM);
+            Erow[i] = 0.5 * m0 * (vx * vx + uzh * uzh);
+            sT += Trow[i]; sE += Erow[i];
+        }
+        const double mT = sT / Lx, mE = sE / Lx;
+        double vT = 0.0, vE = 0.0;
+        for (int i = 0; i < Lx; ++i) {
+            vT += (Trow[i] - mT) * (Trow[i] - mT);
+            vE += (Erow[i] - mE) * (Erow[i] - mE);
+        }
+        if (Tbar) Tbar[k] = mT;
+        if (Trms) Trms[k] = sqrt(vT / Lx);
+        if (Ekbar) Ekbar[k] = mE;
+        if (Ekrms) Ekrms[k] = sqrt(vE / Lx);
+    }
+    free(Trow); free(Erow);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Growth rate from a logged mixing length, eq. 11 / 14:
+ *   [dL/dt]^2 = 4 alpha g At L   =>   alpha(t_j) = (dL/dt)_j^2 / (4 g At L_j),
+ * "local in time".  dL/dt by centred differences on the (possibly non-uniform)
+ * sample times, one-sided at the two ends.  For the double front pass L_tot and the total At
+ * (alpha_tot of eq. 14).  alpha_j = 0 where L_j <= 0.
+ * ------------------------------------------------------------------------------------- */
+void orc_growth_rate(int n, const double *t, const double *L, double g, double At, double *alpha)
+{
+    for (int j = 0; j < n; ++j) {
+        const int a = j > 0 ? j - 1 : j, b = j < n - 1 ? j + 1 : j;
+        const double dLdt = (b > a) ? (L[b] - L[a]) / (t[b] - t[a]) : 0.0;
+        alpha[j] = L[j] > 0.0 ? dLdt * dLdt / (4.0 * g * At * L[j]) : 0.0;
+    }
+}

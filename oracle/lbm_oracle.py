@@ -61,6 +61,8 @@ def lib():
             + [C.c_double] * 6
             + [C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         )
+        L.orc_profiles.argtypes = [_dp, C.c_int, C.c_int, C.c_double] + [C.c_void_p] * 4
+        L.orc_growth_rate.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_double, _dp]
         _lib = L
     return _lib
 
@@ -171,3 +173,20 @@ def init_rt(Lx, Lz, g, seed, T_d, T_m, T_u, rho_m=1.0, delta=0.0, smooth_w=2.5, 
     lib().orc_init_rt(f, Lx, Lz, g, seed, T_d, T_m, T_u, rho_m, delta, smooth_w, pert_kind, n_modes, amp_lo,
                       amp_hi, rho0.ctypes.data if return_fields else None, T0.ctypes.data if return_fields else None)
     return (f, rho0, T0) if return_fields else f
+
+
+def profiles(f: np.ndarray, g: float):
+    """(Tbar, Trms, Ekbar, Ekrms), each [Lz]: x-means and x-fluctuations of T^(H) and E_k = rho |u^(H)|^2 / 2."""
+    _, Lz, Lx = f.shape
+    outs = [np.empty(Lz) for _ in range(4)]
+    lib().orc_profiles(f, Lx, Lz, g, *[o.ctypes.data for o in outs])
+    return tuple(outs)
+
+
+def growth_rate(t, L, g: float, At: float) -> np.ndarray:
+    """alpha(t_j) = (dL/dt)^2 / (4 g At L), eq. 11 / 14."""
+    t = np.ascontiguousarray(t, np.float64)
+    L = np.ascontiguousarray(L, np.float64)
+    out = np.empty(len(t))
+    lib().orc_growth_rate(len(t), t, L, g, At, out)
+    return out
