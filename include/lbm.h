@@ -109,6 +109,19 @@ int lbm_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *
 int lbm_mixing_widths(lbm_t *h, double T_d, double T_m, double T_u, double *L_u, double *L_d, double *Tbar,
                       void *stream);
 
+/* Row profiles of section IV from the hydrodynamic fields of the stored state: Tbar(k) = <T^(H)>_x
+ * (PAPER.md:128), Trms(k) = sqrt(<(T - <T>_x)^2>_x) (Fig. 8), and the same two for the kinetic
+ * energy density E_k = rho |u^(H)|^2 / 2 (Fig. 9; reading 17).  HOST arrays [Lz], any
+ * may be NULL.  Synchronises `stream`. */
+int lbm_profiles(lbm_t *h, double *Tbar, double *Trms, double *Ekbar, double *Ekrms, void *stream);
+
+/* Growth rate from a logged mixing length (host-only post-processing, no device work): eq. 11 / 14
+ * (PAPER.md:169, 199-202), alpha_j = (dL/dt)_j^2 / (4 g At L_j), dL/dt by centred differences on the sample
+ * times t[0..n) (one-sided at both ends), alpha_j = 0 where L_j <= 0.  For the double front pass
+ * L_tot = L_u + L_d and the total Atwood number.  HOST arrays.  Errors: null series, g <= 0, At <= 0,
+ * non-increasing times. */
+int lbm_growth_rate(int n, const double *t, const double *L, double g, double At, double *alpha);
+
 /* Lattice totals sum f, sum c_x f, sum c_z f, sum |c|^2 f into HOST out[4] (deterministic two-stage
  * reduction). Synchronises `stream`. */
 int lbm_totals(lbm_t *h, double *out4, void *stream);

@@ -11,7 +11,7 @@ import ctypes as C
 from . import binding
 from .binding import LbmError, NPOP, lbm_params, lbm_rt_init
 
-__all__ = ["Lattice", "LbmError", "NPOP", "buffer_bytes", "tables"]
+__all__ = ["Lattice", "LbmError", "NPOP", "buffer_bytes", "tables", "growth_rate"]
 
 
 def buffer_bytes(Lx: int, Lz: int) -> int:
@@ -23,6 +23,16 @@ def tables():
     ex, ez, w, r = (C.c_int * NPOP)(), (C.c_int * NPOP)(), (C.c_double * NPOP)(), C.c_double()
     binding.check(binding.load().lbm_tables(ex, ez, w, C.byref(r)))
     return list(ex), list(ez), list(w), r.value
+
+
+def growth_rate(t, L, g: float, At: float):
+    """alpha(t_j) of eq. 11 / 14 from a logged mixing length (lbm_growth_rate; host-only)."""
+    import numpy as np
+    t = np.ascontiguousarray(t, np.float64)
+    L = np.ascontiguousarray(L, np.float64)
+    out = np.empty(len(t))
+    binding.check(binding.load().lbm_growth_rate(len(t), t.ctypes.data, L.ctypes.data, g, At, out.ctypes.data))
+    return out
 
 
 def _stream_ptr(stream):
@@ -113,6 +123,13 @@ class Lattice:
         binding.check(self._lib.lbm_mixing_widths(self._h, T_d, T_m, T_u, C.byref(lu), C.byref(ld),
                                                   tbar.ctypes.data if want_tbar else None, _stream_ptr(stream)))
         return lu.value, ld.value, tbar
+
+    def profiles(self, stream=None):
+        """(Tbar, Trms, Ekbar, Ekrms), host numpy arrays [Lz] (lbm_profiles)."""
+        import numpy as np
+        outs = [np.empty(self.Lz) for _ in range(4)]
+        binding.check(self._lib.lbm_profiles(self._h, *[o.ctypes.data for o in outs], _stream_ptr(stream)))
+        return tuple(outs)
 
     def totals(self, stream=None):
         import numpy as np

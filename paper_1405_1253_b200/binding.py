@@ -17,7 +17,7 @@ NPOP = 37
 SYMBOLS = [
     "lbm_buffer_bytes", "lbm_create", "lbm_destroy", "lbm_init_rt", "lbm_init_equilibrium",
     "lbm_set_populations", "lbm_get_populations", "lbm_set_populations_host", "lbm_get_populations_host",
-    "lbm_step", "lbm_moments", "lbm_mixing_widths", "lbm_totals", "lbm_run_host", "lbm_steps_done",
+    "lbm_step", "lbm_moments", "lbm_mixing_widths", "lbm_profiles", "lbm_growth_rate", "lbm_totals", "lbm_run_host", "lbm_steps_done",
     "lbm_layout", "lbm_kernel_launches", "lbm_set_variant", "lbm_tables", "lbm_last_error",
 ]
 
@@ -62,6 +62,8 @@ def load():
     L.lbm_step.argtypes = [vp, C.c_int, vp]
     L.lbm_moments.argtypes = [vp, vp, vp, vp, vp, vp]
     L.lbm_mixing_widths.argtypes = [vp, C.c_double, C.c_double, C.c_double, dp, dp, vp, vp]
+    L.lbm_profiles.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.lbm_growth_rate.argtypes = [C.c_int, vp, vp, C.c_double, C.c_double, vp]
     L.lbm_totals.argtypes = [vp, dp, vp]
     L.lbm_run_host.argtypes = [vp, vp, vp, vp, vp, C.c_int, vp, vp, vp, vp, vp]
     L.lbm_steps_done.argtypes = [vp, C.POINTER(C.c_longlong)]

@@ -298,6 +298,36 @@ int lbm_mixing_widths(lbm_t *h, double T_d, double T_m, double T_u, double *L_u,
     return LBM_OK;
 }
 
+int lbm_profiles(lbm_t *h, double *Tbar, double *Trms, double *Ekbar, double *Ekrms, void *stream)
+{
+    NEED(h);
+    cudaStream_t st = (cudaStream_t)stream;
+    double *d = h->d_partial();  // [4][Lz], shared with the totals partials
+    lbm::row_profiles_kernel<<<h->Lz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, d);
+    LAUNCHED(h);
+    double *out[4] = {Tbar, Trms, Ekbar, Ekrms};
+    for (int j = 0; j < 4; ++j)
+        if (out[j]) CUDA_TRY(cudaMemcpyAsync(out[j], d + (long long)j * h->Lz, sizeof(double) * h->Lz, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return LBM_OK;
+}
+
+int lbm_growth_rate(int n, const double *t, const double *L, double g, double At, double *alpha)
+{
+    if (n < 0 || (n > 0 && (!t || !L || !alpha))) return fail(LBM_ERR_INVALID, "lbm_growth_rate: null series");
+    if (!(g > 0.0) || !(At > 0.0)) return fail(LBM_ERR_INVALID, "lbm_growth_rate: g and At must be > 0");
+    for (int j = 0; j < n; ++j) {
+        const int lo = j == 0 ? 0 : j - 1, hi = j == n - 1 ? j : j + 1;
+        double slope = 0.0;
+        if (hi > lo) {
+            if (!(t[hi] > t[lo])) return fail(LBM_ERR_INVALID, "lbm_growth_rate: times must increase");
+            slope = (L[hi] - L[lo]) / (t[hi] - t[lo]);
+        }
+        alpha[j] = L[j] > 0.0 ? (slope * slope) / (4.0 * g * At * L[j]) : 0.0;
+    }
+    return LBM_OK;
+}
+
 int lbm_totals(lbm_t *h, double *out4, void *stream)
 {
     NEED(h);

@@ -148,6 +148,48 @@ __global__ void __launch_bounds__(RED_T) row_tbar_kernel(const double *__restric
     if (threadIdx.x == 0) Tbar[k] = t / (double)g.Lx;
 }
 
+// Row profiles of section IV (Fig. 8, Fig. 9): x-mean and x-rms of
+// T^(H) and of E_k = rho |u^(H)|^2 / 2 (reading 17).  One block per row, two passes (means, then
+// squared deviations; the second pass re-reads the row from L2), deterministic.  out = [4][Lz]:
+// Tbar | Trms | Ekbar | Ekrms.
+__global__ void __launch_bounds__(RED_T) row_profiles_kernel(const double *__restrict__ src, Layout g, double grav, double *out)
+{
+    __shared__ double sm[RED_T / 32];
+    __shared__ double mean[2];
+    const int k = blockIdx.x;
+    double aT = 0.0, aE = 0.0;
+    for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
+        double f[NPOP];
+        load_site(src, g, i, k, f);
+        const d2q37::Kinetic m = d2q37::kinetic_moments(f);
+        const double uz = m.uz + 0.5 * grav;
+        aT += m.T + 0.125 * grav * grav;
+        aE += 0.5 * m.rho * (m.ux * m.ux + uz * uz);
+    }
+    const double sT = block_sum(aT, sm), sE = block_sum(aE, sm);
+    if (threadIdx.x == 0) { mean[0] = sT / (double)g.Lx; mean[1] = sE / (double)g.Lx; }
+    __syncthreads();
+    const double mT = mean[0], mE = mean[1];
+    double vT = 0.0, vE = 0.0;
+    for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
+        double f[NPOP];
+        load_site(src, g, i, k, f);
+        const d2q37::Kinetic m = d2q37::kinetic_moments(f);
+        const double uz = m.uz + 0.5 * grav;
+        const double dT = m.T + 0.125 * grav * grav - mT;
+        const double dE = 0.5 * m.rho * (m.ux * m.ux + uz * uz) - mE;
+        vT += dT * dT;
+        vE += dE * dE;
+    }
+    const double qT = block_sum(vT, sm), qE = block_sum(vE, sm);
+    if (threadIdx.x == 0) {
+        out[k] = mT;
+        out[g.Lz + k] = sqrt(qT / (double)g.Lx);
+        out[2 * g.Lz + k] = mE;
+        out[3 * g.Lz + k] = sqrt(qE / (double)g.Lx);
+    }
+}
+
 // tent map of eq. 9, zero outside (0,1)
 __device__ __forceinline__ double tent(double b)
 {

@@ -4,7 +4,7 @@
     python -m paper_1405_1253_b200.run_rt --config 2 [--steps N] [--every 100] [--out widths.csv]
 
 Every `--every` steps it calls lbm_mixing_widths (eq. 12) and lbm_totals and writes
-step, t/tau_RT, L_u, L_d, L_tot, mass, with tau_RT = sqrt(Lx / (g At)) and
+step, t/tau_RT, L_u, L_d, L_tot, mass, alpha_tot (eq. 14 via lbm_growth_rate), with tau_RT = sqrt(Lx / (g At)) and
 At = (T_d - T_u)/(T_d + T_u) (Table II).  All arithmetic runs in the CUDA library.
 """
 from __future__ import annotations
@@ -36,11 +36,7 @@ def run(cfg, steps: int, every: int, seed: int = si.DEFAULT_SEED, out=None, vari
         lu, ld, _ = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)
         mass = lat.totals()[0]
         rows.append((lat.steps_done, lat.steps_done / tau_rt, lu, ld, lu + ld, mass))
-        if out:
-            out.write("%d,%.6f,%.9f,%.9f,%.9f,%.15e\n" % rows[-1])
 
-    if out:
-        out.write("step,t_over_tau,L_u,L_d,L_tot,mass\n")
     log()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -53,6 +49,9 @@ def run(cfg, steps: int, every: int, seed: int = si.DEFAULT_SEED, out=None, vari
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
     lat.close()
+    # alpha_tot(t) of eq. 14 from the logged L_tot; appended as a 7th column
+    alpha = pkg.growth_rate([r[0] for r in rows], [r[4] for r in rows], cfg.g, At) if len(rows) > 1 and cfg.g > 0 else [0.0] * len(rows)
+    rows = [r + (float(a),) for r, a in zip(rows, alpha)]
     return rows, wall
 
 
@@ -67,8 +66,11 @@ def main():
     cfg = si.rt_config(args.config)
     steps = args.steps or cfg.steps
     fh = open(args.out, "w") if args.out else None
-    rows, wall = run(cfg, steps, args.every, args.seed, fh)
+    rows, wall = run(cfg, steps, args.every, args.seed)
     if fh:
+        fh.write("step,t_over_tau,L_u,L_d,L_tot,mass,alpha_tot\n")
+        for r in rows:
+            fh.write("%d,%.6f,%.9f,%.9f,%.9f,%.15e,%.6e\n" % r)
         fh.close()
     sites = cfg.Lx * cfg.Lz
     print(f"{cfg.name}: {steps} steps in {wall:.2f} s incl. {len(rows)} diagnostics = "

@@ -158,3 +158,41 @@ def test_run_host_end_to_end(pkg, orc):
     for o, r_ in zip(outs, ref):
         assert np.max(np.abs(o.numpy() - r_)) < 1e-13
     lat.close()
+
+
+def test_section4_profiles_match_oracle(pkg, orc):
+    """Fluctuation profiles of Fig. 8-9 (lbm_profiles) on an evolved RT state, row by row."""
+    cfg = si.scaled(si.rt_config(2), 200, 96)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, 2e-3)       # strong gravity so that the half-step shifts matter
+    lat.init_rt(5, **cfg.rt_args())
+    lat.step(30)
+    ref = orc.step(orc.init_rt(cfg.Lx, cfg.Lz, 2e-3, 5, **cfg.rt_args()), cfg.tau, 2e-3, nsteps=30)
+    got, want = lat.profiles(), orc.profiles(ref, 2e-3)
+    for a, b, tol in zip(got, want, (1e-13, 1e-12, 1e-16, 1e-15)):
+        assert np.max(np.abs(a - b)) < tol
+    assert want[1].max() > 1e-4 and want[3].max() > 1e-9      # the profiles are not trivially zero
+    assert np.max(np.abs(got[0] - lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u)[2])) < 1e-14
+    lat.close()
+
+
+def test_step_is_cuda_graph_capturable(pkg):
+    """lbm_step only enqueues kernels on the given stream, so an even number of steps can be captured in a
+    CUDA graph and replayed (the ping-pong returns to the same buffers)."""
+    import torch
+    Lx, Lz = 96, 64
+    fields = [torch.from_numpy(x).cuda() for x in si.sweep_fields(Lx, Lz, seed=4)]
+    a, b = pkg.Lattice(Lx, Lz, 0.8, 1e-4), pkg.Lattice(Lx, Lz, 0.8, 1e-4)
+    a.init_equilibrium(*fields); b.init_equilibrium(*fields)
+    a.step(10)                                            # 2 warm-up + 4 replays x 2; capture itself runs nothing
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        b.step(2, stream=s)                                   # warm-up outside capture
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            b.step(2, stream=s)
+        for _ in range(4):
+            graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(a.get_populations(), b.get_populations())
+    a.close(); b.close()

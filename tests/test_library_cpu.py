@@ -93,3 +93,19 @@ def test_synthetic_inputs_are_reproducible_and_sliceable():
     cfg = si.rt_config(4)
     assert (cfg.Lx, cfg.Lz, cfg.delta, cfg.pert_kind) == (4096, 8192, 0.0, si.PERT_WHITE)
     assert si.scaled(si.rt_config(2), 128, 256).delta == 64
+
+
+def test_growth_rate_host_function_matches_oracle_and_closed_form(lib, orc):
+    """lbm_growth_rate is host-only post-processing (eq. 11 / 14), so it is checked here without a GPU."""
+    import paper_1405_1253_b200 as pkg
+    rng = np.random.default_rng(8)
+    t = np.cumsum(rng.uniform(50, 150, 30))
+    L = 0.05 * 1.5e-5 * 0.025 * t ** 2 * (1 + 0.1 * np.sin(t / 300))
+    a, b = pkg.growth_rate(t, L, 1.5e-5, 0.025), orc.growth_rate(t, L, 1.5e-5, 0.025)
+    assert np.max(np.abs(a - b)) <= 1e-15 * np.max(np.abs(b))
+    tq = np.arange(1, 20) * 100.0
+    assert np.max(np.abs(pkg.growth_rate(tq, 0.04 * 1e-4 * 0.05 * tq ** 2, 1e-4, 0.05)[1:-1] / 0.04 - 1)) < 1e-12
+    with pytest.raises(pkg.LbmError):
+        pkg.growth_rate(tq[::-1].copy(), tq, 1e-4, 0.05)      # times must increase
+    with pytest.raises(pkg.LbmError):
+        pkg.growth_rate(tq, tq, 0.0, 0.05)
