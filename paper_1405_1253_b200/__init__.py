@@ -171,6 +171,9 @@ class Lattice:
     def set_variant(self, variant: int):
         binding.check(self._lib.lbm_set_variant(self._h, int(variant)))
 
+    def set_zchunk(self, rows: int):
+        binding.check(self._lib.lbm_set_zchunk(self._h, int(rows)))
+
     # ---- argument checks (marshalling only)
     def _check_fields(self, *fields):
         import torch

@@ -13,6 +13,7 @@
 #include "../../include/lbm.h"
 #include "lbm_aux.cuh"
 #include "lbm_step.cuh"
+#include "lbm_step2.cuh"
 
 namespace {
 
@@ -78,6 +79,7 @@ struct lbm_handle {
     int cur;               // index of the current lattice
     long long steps, launches;
     int variant;
+    int zchunk;            // rows per block of the two-step kernel (multiple of S2_R)
     double *scratch;       // device: Tbar[Lz] | row partials[4 Lz] | results[8] | h_lo[Lx] | h_hi[Lx]
     double *stage[4];      // device staging fields for lbm_run_host (lazy)
     lbm::Layout layout() const { return lbm::Layout{Lx, Lz, pitch, plane}; }
@@ -139,7 +141,7 @@ int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p)
     h->Lx = Lx; h->Lz = Lz; h->pitch = pitch_of(Lx); h->plane = plane_of(Lx, Lz);
     h->tau = p->tau; h->g = p->g;
     h->buf[0] = (double *)p->pop_buf0; h->buf[1] = (double *)p->pop_buf1;
-    h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->scratch = nullptr;
+    h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 192; h->scratch = nullptr;
     for (auto &s : h->stage) s = nullptr;
     cudaError_t e = cudaMalloc(&h->scratch, sizeof(double) * (5LL * Lz + 8 + 2LL * Lx));
     if (e != cudaSuccess) { delete h; return fail(LBM_ERR_CUDA, "lbm_create: cudaMalloc scratch: %s", cudaGetErrorString(e)); }
@@ -252,7 +254,25 @@ int lbm_step(lbm_t *h, int n, void *stream)
     a.omega = 1.0 / h->tau;
     a.gtau = h->g * h->tau;
     a.dT = 0.5 * h->tau * (1.0 - h->tau) * h->g * h->g;
-    for (int s = 0; s < n; ++s) {
+    int s = 0;
+    if (h->variant == 3) {  // two steps per launch (lbm_step2.cuh); an odd last step falls through
+        static bool attr_set = false;
+        if (!attr_set) {
+            CUDA_TRY(cudaFuncSetAttribute(lbm::step2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lbm::S2_SMEM));
+            attr_set = true;
+        }
+        const int ZC = h->zchunk;
+        dim3 grid((h->Lx + lbm::S2_TX - 1) / lbm::S2_TX, (h->Lz + ZC - 1) / ZC);
+        for (; s + 2 <= n; s += 2) {
+            a.src = h->buf[h->cur];
+            a.dst = h->buf[h->cur ^ 1];
+            lbm::step2_kernel<<<grid, lbm::S2_THREADS, lbm::S2_SMEM, st>>>(a, ZC);
+            LAUNCHED(h);
+            h->cur ^= 1;
+            h->steps += 2;
+        }
+    }
+    for (; s < n; ++s) {
         a.src = h->buf[h->cur];
         a.dst = h->buf[h->cur ^ 1];
         switch (h->variant) {
@@ -389,10 +409,18 @@ int lbm_kernel_launches(const lbm_t *h, long long *launches)
     return LBM_OK;
 }
 
+int lbm_set_zchunk(lbm_t *h, int rows)
+{
+    NEED(h);
+    if (rows < lbm::S2_R || rows % lbm::S2_R) return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be a positive multiple of %d (got %d)", lbm::S2_R, rows);
+    h->zchunk = rows;
+    return LBM_OK;
+}
+
 int lbm_set_variant(lbm_t *h, int variant)
 {
     NEED(h);
-    if (variant < 0 || variant > 2) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
+    if (variant < 0 || variant > 3) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
     h->variant = variant;
     return LBM_OK;
 }

@@ -1,0 +1,127 @@
+// lbm_step2.cuh -- TWO time steps per launch (temporal blocking): propagate+bc+collide, twice, with the
+// intermediate lattice kept in shared memory, so that HBM sees ~296 B read + 296 B written per site per TWO
+// steps instead of per step.
+//
+// A block owns a strip of S2_TX = 64 output columns and marches up a chunk of ZC rows.  It keeps a ring of
+// S2_RING = 9 rows of the INTERMEDIATE state f1 = step(f0) for the S2_TX + 6 columns x0-3 .. x0+66 (the three
+// halo columns per side are recomputed redundantly instead of exchanged: +9 % first-step work, and their
+// source sectors are shared with the neighbouring strip through L2).  Per iteration of S2_R = 3 rows:
+//   A  (first step, PAPER.md:114 propagate+bc+collide): every thread owns one site of 3 new f1 rows, gathers its
+//      37 populations from the global source lattice (periodic wrap + wall remap exactly as in lbm_step.cuh),
+//      collides in registers and stores the 37 results into the ring;
+//   B  (second step): every thread owns one site of 3 output rows, gathers its 37 populations from the ring
+//      (rows k-3..k+3, wall remap, no wrap needed: ring columns are strip-local), collides, and writes f2 to the
+//      global destination lattice with aligned stores.
+// The global loads of the NEXT A pass are issued before B starts and are consumed after it, so HBM latency is
+// hidden behind B's arithmetic with a single resident block per SM.  Arithmetic is the same collide_site() as
+// the one-step kernel, so two fused steps are bit-identical to two single steps (tested).
+#pragma once
+#include "lbm_step.cuh"
+
+namespace lbm {
+
+constexpr int S2_TX = 64;                 // output columns per strip
+constexpr int S2_W1 = S2_TX + 6;          // intermediate columns per strip
+constexpr int S2_CP = 72;                 // shared-memory row pitch (doubles)
+constexpr int S2_R = 3;                   // rows per iteration
+constexpr int S2_RING = S2_R + 6;         // intermediate rows resident
+constexpr int S2_THREADS = 256;           // 8 warps: 210 lanes for A (3 x 70 sites), 192 for B (3 x 64);
+                                          // 256 threads may use up to 255 registers (prefetch + working set)
+constexpr size_t S2_SMEM = sizeof(double) * S2_RING * NPOP * S2_CP;   // 191 808 B
+
+// Second-step gather of output site (strip column bj, row k) from the ring of intermediate rows.
+template <bool WALL>
+__device__ __forceinline__ void gather_ring(const double *ring, int Lz, int z0, int bj, int k, double (&f)[NPOP])
+{
+    int rowoff[7];
+    bool flip[7];
+#pragma unroll
+    for (int d = -3; d <= 3; ++d) {
+        int ks = k - d;
+        bool fl = false;
+        if (WALL) {
+            if (ks < 0) { ks = -1 - ks; fl = true; }
+            else if (ks >= Lz) { ks = 2 * Lz - 1 - ks; fl = true; }
+        }
+        rowoff[d + 3] = ((ks - z0 + 3) % S2_RING) * (NPOP * S2_CP);
+        flip[d + 3] = fl;
+    }
+    const double *q = ring + bj + 3;
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        constexpr int ex = d2q37::pop_ex(l), ez = d2q37::pop_ez(l);
+        int ls = l;
+        if (WALL) ls = flip[ez + 3] ? (NPOP - 1 - l) : l;
+        f[l] = q[rowoff[ez + 3] + ls * S2_CP - ex];
+    });
+}
+
+__global__ void __launch_bounds__(S2_THREADS, 1) step2_kernel(const StepArgs a, const int ZC)
+{
+    extern __shared__ double ring[];      // [S2_RING][NPOP][S2_CP]
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * S2_TX, z0 = blockIdx.y * ZC;
+    const int ncols = min(S2_TX, a.Lx - x0);          // output columns of this strip
+    const int zend = min(a.Lz, z0 + ZC);               // output rows [z0, zend)
+    const int rlast = min(a.Lz, zend + 3);             // intermediate rows [max(0, z0-3), rlast)
+
+    // A mapping: thread -> (row within pass, strip-local column), global column wrapped once
+    const int ar = tid / S2_W1, aj = tid - ar * S2_W1;
+    const bool a_lane = tid < S2_R * S2_W1 && aj < ncols + 6;
+    int ac = (x0 - 3 + aj) % a.Lx;
+    if (ac < 0) ac += a.Lx;
+    // B mapping
+    const int br = tid >> 6, bj = tid & 63;
+    const bool b_lane = tid < S2_R * S2_TX && bj < ncols;
+
+    double g[NPOP];                                    // inputs of the pending A pass
+
+    auto a_valid = [&](int row0, int nrows) {
+        const int r = row0 + ar;
+        return a_lane && ar < nrows && r >= 0 && r < rlast;
+    };
+    auto a_issue = [&](int row0, int nrows) {          // first step, gather part: loads stay in flight
+        if (a_valid(row0, nrows)) {
+            const int r = row0 + ar;
+            if (r >= 3 && r < a.Lz - 3) gather_site<false>(a, ac, r, g);
+            else gather_site<true>(a, ac, r, g);
+        }
+    };
+    auto a_finish = [&](int row0, int nrows) {         // first step, collide part: results into the ring
+        if (a_valid(row0, nrows)) {
+            const int r = row0 + ar;
+            d2q37::collide_site(g, a.omega, a.gtau, a.dT);
+            double *p = ring + ((r - z0 + 3) % S2_RING) * (NPOP * S2_CP) + aj;
+            d2q37::static_for<0, NPOP>([&](auto L) {
+                constexpr int l = decltype(L)::value;
+                p[l * S2_CP] = g[l];
+            });
+        }
+    };
+
+    // warm-up: intermediate rows z0-3 .. z0+2
+    static_assert(S2_R == 3, "the warm-up below issues two passes of three rows");
+    a_issue(z0 - 3, S2_R);
+    a_finish(z0 - 3, S2_R);
+    a_issue(z0, S2_R);
+    a_finish(z0, S2_R);
+    a_issue(z0 + 3, S2_R);
+
+    for (int k0 = z0; k0 < zend; k0 += S2_R) {
+        a_finish(k0 + 3, S2_R);                        // intermediate rows k0+3 .. k0+6
+        __syncthreads();
+        if (k0 + S2_R < zend) a_issue(k0 + S2_R + 3, S2_R);   // prefetch the next pass behind B
+
+        const int k = k0 + br;
+        if (b_lane && k < zend) {
+            double f[NPOP];
+            if (k >= 3 && k < a.Lz - 3) gather_ring<false>(ring, a.Lz, z0, bj, k, f);
+            else gather_ring<true>(ring, a.Lz, z0, bj, k, f);
+            d2q37::collide_site(f, a.omega, a.gtau, a.dT);
+            scatter_site(a, x0 + bj, k, f);
+        }
+        __syncthreads();                               // B has read the rows the next A pass overwrites
+    }
+}
+
+}  // namespace lbm
