@@ -176,6 +176,8 @@ def run_ours(args):
     lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
     if args.variant is not None:
         lat.set_variant(args.variant)
+    if args.zchunk:
+        lat.set_zchunk(args.zchunk)
     lat.init_rt(si.DEFAULT_SEED + rank, **cfg.rt_args())     # replicas differ only by their seed
 
     def barrier():
@@ -275,6 +277,8 @@ def run_sweep(args):
         lat = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G)
         for v in variants:
             lat.set_variant(v)
+            if args.zchunk:
+                lat.set_zchunk(args.zchunk)
             lat.init_equilibrium(*fields)
             lat.step(args.warmup)
             torch.cuda.synchronize()
@@ -285,7 +289,7 @@ def run_sweep(args):
             t = e0.elapsed_time(e1) * 1e-3 / args.steps
             tm = e1.elapsed_time(e2) * 1e-3
             tot = lat.totals()
-            print(json.dumps({"sweep": f"{Lx}x{Lz}", "variant": v, "mlups": sites / t / 1e6, "us_per_step": t * 1e6,
+            print(json.dumps({"sweep": f"{Lx}x{Lz}", "variant": v, "zchunk": args.zchunk, "mlups": sites / t / 1e6, "us_per_step": t * 1e6,
                               "gbs": BYTES_PER_SITE * sites / t / 1e9, "frac_of_measured_peak": BYTES_PER_SITE * sites / t / 1e9 / peak,
                               "resident": "L2" if 2 * 37 * 8 * sites < 126e6 else "HBM",
                               "moments_gbs": 328 * sites / tm / 1e9, "mass": tot[0]}), flush=True)
@@ -305,6 +309,7 @@ def main():
     ap.add_argument("--lx", type=int, default=0)
     ap.add_argument("--lz", type=int, default=0)
     ap.add_argument("--variant", type=int, default=None, help="step-kernel variant (default: library default)")
+    ap.add_argument("--zchunk", type=int, default=0, help="rows per block of the two-step kernel (multiple of 3)")
     ap.add_argument("--e2e-steps", type=int, default=0)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

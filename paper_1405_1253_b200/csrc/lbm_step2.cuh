@@ -13,7 +13,10 @@
 //      (rows k-3..k+3, wall remap, no wrap needed: ring columns are strip-local), collides, and writes f2 to the
 //      global destination lattice with aligned stores.
 // The global loads of the NEXT A pass are issued before B starts and are consumed after it, so HBM latency is
-// hidden behind B's arithmetic with a single resident block per SM.  Arithmetic is the same collide_site() as
+// hidden behind B's arithmetic with a single resident block per SM.  The two hand-offs per iteration are split
+// mbarriers (arrive early, wait late): FULL = "this pass's rows are in the ring" (arrive after the stores, wait
+// before B's gather), EMPTY = "B has read the ring" (arrive right after B's gather, wait only before the next
+// pass's stores, i.e. after two collisions), so warps do not rendezvous twice per iteration.  Arithmetic is the same collide_site() as
 // the one-step kernel, so two fused steps are bit-identical to two single steps (tested).
 #pragma once
 #include "lbm_step.cuh"
@@ -28,6 +31,24 @@ constexpr int S2_RING = S2_R + 6;         // intermediate rows resident
 constexpr int S2_THREADS = 256;           // 8 warps: 210 lanes for A (3 x 70 sites), 192 for B (3 x 64);
                                           // 256 threads may use up to 255 registers (prefetch + working set)
 constexpr size_t S2_SMEM = sizeof(double) * S2_RING * NPOP * S2_CP;   // 191 808 B
+
+// split-phase block barrier on an mbarrier in shared memory (all S2_THREADS threads arrive on every phase)
+__device__ __forceinline__ void mbar_init(unsigned bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
 
 // Second-step gather of output site (strip column bj, row k) from the ring of intermediate rows.
 template <bool WALL>
@@ -99,6 +120,12 @@ __global__ void __launch_bounds__(S2_THREADS, 1) step2_kernel(const StepArgs a, 
         }
     };
 
+    __shared__ unsigned long long bars[2];
+    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(&bars[0]);
+    const unsigned bar_empty = (unsigned)__cvta_generic_to_shared(&bars[1]);
+    if (tid == 0) { mbar_init(bar_full, S2_THREADS); mbar_init(bar_empty, S2_THREADS); }
+    __syncthreads();
+
     // warm-up: intermediate rows z0-3 .. z0+2
     static_assert(S2_R == 3, "the warm-up below issues two passes of three rows");
     a_issue(z0 - 3, S2_R);
@@ -107,20 +134,36 @@ __global__ void __launch_bounds__(S2_THREADS, 1) step2_kernel(const StepArgs a, 
     a_finish(z0, S2_R);
     a_issue(z0 + 3, S2_R);
 
-    for (int k0 = z0; k0 < zend; k0 += S2_R) {
-        a_finish(k0 + 3, S2_R);                        // intermediate rows k0+3 .. k0+6
-        __syncthreads();
+    unsigned phase = 0;
+    for (int k0 = z0; k0 < zend; k0 += S2_R, phase ^= 1) {
+        // first step of rows k0+3 .. k0+5: collide, then store once B of the previous iteration has read the ring
+        const bool av = a_valid(k0 + 3, S2_R);
+        if (av) d2q37::collide_site(g, a.omega, a.gtau, a.dT);
+        if (k0 > z0) mbar_wait(bar_empty, phase ^ 1);
+        if (av) {
+            double *p = ring + ((k0 + ar + 6 - z0) % S2_RING) * (NPOP * S2_CP) + aj;
+            d2q37::static_for<0, NPOP>([&](auto L) {
+                constexpr int l = decltype(L)::value;
+                p[l * S2_CP] = g[l];
+            });
+        }
+        mbar_arrive(bar_full);
         if (k0 + S2_R < zend) a_issue(k0 + S2_R + 3, S2_R);   // prefetch the next pass behind B
+        mbar_wait(bar_full, phase);
 
+        // second step of rows k0 .. k0+2
         const int k = k0 + br;
-        if (b_lane && k < zend) {
-            double f[NPOP];
+        const bool bv = b_lane && k < zend;
+        double f[NPOP];
+        if (bv) {
             if (k >= 3 && k < a.Lz - 3) gather_ring<false>(ring, a.Lz, z0, bj, k, f);
             else gather_ring<true>(ring, a.Lz, z0, bj, k, f);
+        }
+        mbar_arrive(bar_empty);
+        if (bv) {
             d2q37::collide_site(f, a.omega, a.gtau, a.dT);
             scatter_site(a, x0 + bj, k, f);
         }
-        __syncthreads();                               // B has read the rows the next A pass overwrites
     }
 }
 
