@@ -254,6 +254,7 @@ int lbm_step(lbm_t *h, int n, void *stream)
     a.omega = 1.0 / h->tau;
     a.gtau = h->g * h->tau;
     a.dT = 0.5 * h->tau * (1.0 - h->tau) * h->g * h->g;
+    lbm::fill_offsets(a);
     int s = 0;
     if (h->variant == 3) {  // two steps per launch (lbm_step2.cuh); an odd last step falls through
         static bool attr_set = false;

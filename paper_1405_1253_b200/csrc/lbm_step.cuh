@@ -27,19 +27,24 @@ struct StepArgs {
     double omega;       // dt / tau
     double gtau;        // g tau
     double dT;          // tau (1 - tau) g^2 / 2
+    // byte offset of population l's pull source relative to the site's own address in plane 0, for sites that
+    // need neither wrap nor wall remap: 8 (l plane - e_lz pitch - e_lx).  Host-computed (fill_offsets) so that
+    // the kernel adds one opaque uniform constant per load instead of re-deriving it.
+    long long gbyte[NPOP];
 };
 
-// streaming load / store: every population value is read once and written once per step
-__device__ __forceinline__ double ld_stream(const double *p)
+inline void fill_offsets(StepArgs &a)
 {
-    double v;
-    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
-    return v;
+    for (int l = 0; l < NPOP; ++l)
+        a.gbyte[l] = 8 * ((long long)l * a.plane - (long long)d2q37::pop_ez(l) * a.pitch - d2q37::pop_ex(l));
 }
-__device__ __forceinline__ void st_stream(double *p, double v)
-{
-    asm volatile("st.global.L1::no_allocate.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
-}
+
+// Streaming load / store: every population value is read once and written once per step.  Plain
+// ld.global.nc / st.global: explicit cache operators (L1::no_allocate, .cs, L2 evict_first) were measured and
+// make no difference (profiles/r1_variants.md), and the builtin forms let the compiler fold the constant part
+// of each address into the instruction's immediate.
+__device__ __forceinline__ double ld_stream(const double *p) { return __ldg(p); }
+__device__ __forceinline__ void st_stream(double *p, double v) { *p = v; }
 
 // Gather the 37 post-propagate populations of site (i, k).  WALL = false: rows 3..Lz-4, no remap.
 template <bool WALL>
@@ -77,6 +82,27 @@ __device__ __forceinline__ void gather_site(const StepArgs &a, int i, int k, dou
     });
 }
 
+// Fast path for sites with 3 <= i < Lx-3 and 3 <= k < Lz-3 (no wrap, no wall): every source address is the
+// site's own address plus an offset that depends on kernel arguments only, so the offsets live in uniform
+// registers and each load costs one 64-bit add (the e_x shift is an immediate).
+__device__ __forceinline__ void gather_interior(const StepArgs &a, int i, int k, double (&f)[NPOP])
+{
+    const char *p = reinterpret_cast<const char *>(a.src + (long long)k * a.pitch + i);
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        f[l] = ld_stream(reinterpret_cast<const double *>(p + a.gbyte[l]));
+    });
+}
+
+// dispatch on the site's position: interior / periodic seam / wall rows
+__device__ __forceinline__ void gather_any(const StepArgs &a, int i, int k, double (&f)[NPOP])
+{
+    const bool bulk_z = k >= 3 && k < a.Lz - 3;
+    if (bulk_z && i >= 3 && i < a.Lx - 3) gather_interior(a, i, k, f);
+    else if (bulk_z) gather_site<false>(a, i, k, f);
+    else gather_site<true>(a, i, k, f);
+}
+
 __device__ __forceinline__ void scatter_site(const StepArgs &a, int i, int k, const double (&f)[NPOP])
 {
     double *p = a.dst + (long long)k * a.pitch + i;
@@ -95,8 +121,7 @@ __global__ void __launch_bounds__(TX *TZ) step_kernel_site(const StepArgs a)
     const int k = blockIdx.y * TZ + threadIdx.y;
     if (i >= a.Lx || k >= a.Lz) return;
     double f[NPOP];
-    if (k >= 3 && k < a.Lz - 3) gather_site<false>(a, i, k, f);
-    else gather_site<true>(a, i, k, f);
+    gather_any(a, i, k, f);
     d2q37::collide_site(f, a.omega, a.gtau, a.dT);
     scatter_site(a, i, k, f);
 }

@@ -103,9 +103,7 @@ __global__ void __launch_bounds__(S2_THREADS, 1) step2_kernel(const StepArgs a, 
     };
     auto a_issue = [&](int row0, int nrows) {          // first step, gather part: loads stay in flight
         if (a_valid(row0, nrows)) {
-            const int r = row0 + ar;
-            if (r >= 3 && r < a.Lz - 3) gather_site<false>(a, ac, r, g);
-            else gather_site<true>(a, ac, r, g);
+            gather_any(a, ac, row0 + ar, g);
         }
     };
     auto a_finish = [&](int row0, int nrows) {         // first step, collide part: results into the ring
