@@ -136,8 +136,10 @@ int lbm_run_host(lbm_t *h, const double *rho_in, const double *ux_in, const doub
 int lbm_steps_done(const lbm_t *h, long long *steps);
 int lbm_layout(const lbm_t *h, int *pitch, long long *plane_stride); /* in doubles */
 int lbm_kernel_launches(const lbm_t *h, long long *launches);       /* kernels launched through this handle */
-int lbm_set_variant(lbm_t *h, int variant);                          /* step-kernel variant */
-int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel (variant 3); multiple of 3 */
+/* Step-kernel variant: 0 automatic (default), 1 one step per launch (256-thread blocks), 2 one step (128),
+ * 3 two steps per launch forced (lbm_step2.cuh).  All give bit-identical results. */
+int lbm_set_variant(lbm_t *h, int variant);
+int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel; a multiple of 3, or 0 = automatic */
 /* D2Q37 tables as the library uses them (host outputs, any may be NULL): e_x[37], e_z[37], w[37], r. */
 int lbm_tables(int *ex, int *ez, double *w, double *r);
 const char *lbm_last_error(void);

@@ -50,6 +50,30 @@ __host__ __device__ constexpr int shell_e2(int slot)
     return slot == 0 ? 0 : slot == 1 ? 1 : slot == 2 ? 2 : slot == 3 ? 4 : slot == 4 ? 5 : slot == 5 ? 8 : slot == 6 ? 9 : 10;
 }
 
+// Per-shell constants of the equilibrium polynomial (see equilibrium_blend_from), kept in the constant bank so
+// that they are instruction operands (c[bank][offset]) rather than 64-bit immediates rebuilt with UMOV pairs.
+struct ShellConst {
+    double k1, k2, k3, k4, k5, w;
+};
+__host__ __device__ constexpr ShellConst shell_const(int slot)
+{
+    const double c2 = D2Q37_R2 * shell_e2(slot);
+    return ShellConst{0.5 * (c2 - 2.0), 0.25 * (4.0 - c2), 0.125 * (c2 * c2 - 8.0 * c2 + 8.0),
+                      0.5 * (c2 - 4.0), 0.25 * (c2 - 6.0), shell_weight(shell_e2(slot))};
+}
+static __constant__ ShellConst c_shell[8] = {shell_const(0), shell_const(1), shell_const(2), shell_const(3),
+                                             shell_const(4), shell_const(5), shell_const(6), shell_const(7)};
+static __constant__ double c_lat[4] = {D2Q37_R, D2Q37_R2, 1.0 / 6.0, 1.0 / 24.0};
+
+// first population (ascending l) with a given e_x / e_z: the accumulators of raw_moments_from start there
+__host__ __device__ constexpr int first_with_ex(int ex)
+{
+    for (int l = 0; l < NPOP; ++l)
+        if (pop_ex(l) == ex) return l;
+    return -1;
+}
+__host__ __device__ constexpr int first_with_ez(int ez) { return row_first(ez); }
+
 // compile-time loop: f(std::integral_constant<int, B>{}), ..., f(<E-1>)
 template <int B, int E, class F>
 __host__ __device__ __forceinline__ void static_for(F &&f)
@@ -63,17 +87,24 @@ __host__ __device__ __forceinline__ void static_for(F &&f)
 // Raw lattice moments of one site in integer-velocity form:
 //   m0 = sum f, jx = sum e_x f, jz = sum e_z f, m2 = sum |e|^2 f.
 // Column sums C[e_x] and row sums R[e_z] are formed first (74 adds), the weighted sums from them.
+// `load(L)` returns population l = L::value (registers, shared memory, ...); it is called once per l, in
+// ascending l, so every caller accumulates in the same order (bit-identical results).
 struct RawMoments {
     double m0, jx, jz, m2;
 };
 
-__device__ __forceinline__ RawMoments raw_moments(const double (&f)[NPOP])
+template <class Load>
+__device__ __forceinline__ RawMoments raw_moments_from(Load &&load)
 {
-    double C[7] = {0, 0, 0, 0, 0, 0, 0}, R[7] = {0, 0, 0, 0, 0, 0, 0};
+    double C[7], R[7];
     static_for<0, NPOP>([&](auto L) {
         constexpr int l = decltype(L)::value;
-        C[pop_ex(l) + 3] += f[l];
-        R[pop_ez(l) + 3] += f[l];
+        constexpr int ex = pop_ex(l), ez = pop_ez(l);
+        const double v = load(L);
+        if constexpr (l == first_with_ex(ex)) C[ex + 3] = v;
+        else C[ex + 3] += v;
+        if constexpr (l == first_with_ez(ez)) R[ez + 3] = v;
+        else R[ez + 3] += v;
     });
     RawMoments m;
     const double c1 = C[4] + C[2], c2 = C[5] + C[1], c3 = C[6] + C[0];
@@ -85,25 +116,31 @@ __device__ __forceinline__ RawMoments raw_moments(const double (&f)[NPOP])
     return m;
 }
 
+__device__ __forceinline__ RawMoments raw_moments(const double (&f)[NPOP])
+{
+    return raw_moments_from([&](auto L) { return f[decltype(L)::value]; });
+}
+
 // Kinetic moments of eq. 7: rho = sum f, rho u = sum c f, d rho T = sum |c-u|^2 f, d = 2,
 // with c = r e:  u = r j / rho,  T = (r^2 m2 / rho - |u|^2) / 2.
 struct Kinetic {
     double rho, ux, uz, T;
 };
 
-__device__ __forceinline__ Kinetic kinetic_moments(const double (&f)[NPOP])
+__device__ __forceinline__ Kinetic kinetic_from_raw(const RawMoments &m)
 {
-    const RawMoments m = raw_moments(f);
     const double inv = 1.0 / m.m0;
     Kinetic k;
     k.rho = m.m0;
-    k.ux = (D2Q37_R * m.jx) * inv;
-    k.uz = (D2Q37_R * m.jz) * inv;
-    k.T = 0.5 * ((D2Q37_R2 * m.m2) * inv - (k.ux * k.ux + k.uz * k.uz));
+    k.ux = (c_lat[0] * m.jx) * inv;
+    k.uz = (c_lat[0] * m.jz) * inv;
+    k.T = 0.5 * ((c_lat[1] * m.m2) * inv - (k.ux * k.ux + k.uz * k.uz));
     return k;
 }
 
-// out[l] = keep * fin[l] + scale * f_eq_l(rho = 1, u, T), for all l.
+__device__ __forceinline__ Kinetic kinetic_moments(const double (&f)[NPOP]) { return kinetic_from_raw(raw_moments(f)); }
+
+// store(L, keep * load(L) + scale * f_eq_l(rho = 1, u, T)) for all l.
 //
 // f_eq is the 4th-order Hermite projection of the Maxwellian on this quadrature ("local Maxwellian",
 // PAPER.md:80; reading 3).  With s = c.u, q = |u|^2, theta = T - 1, D = 2 it is a quartic in s
@@ -112,12 +149,14 @@ __device__ __forceinline__ Kinetic kinetic_moments(const double (&f)[NPOP])
 //   g0 = 1 - q/2 + q^2/8 + theta [ (c2-2)/2 + q (4-c2)/4 ] + theta^2 (c2^2 - 8 c2 + 8)/8
 //   g1 = 1 - q/2 + theta (c2-4)/2
 //   g2 = 1/2 - q/4 + theta (c2-6)/4
-// so each population costs one Horner evaluation (4 FMA) plus the relaxation FMA.
-//   collision (rhs of eq. 5): keep = 1 - 1/tau, scale = rho/tau, fin = post-propagate f
+// so each population costs one Horner evaluation (4 FMA) plus the relaxation FMA.  Shells are the outer
+// loop: only one shell's five coefficients are live at a time (register pressure), and every population's
+// value is the same expression whichever order the populations are visited in.
+//   collision (rhs of eq. 5): keep = 1 - 1/tau, scale = rho/tau, load = post-propagate f
 //   plain equilibrium:                      keep = 0,         scale = rho
-template <bool KEEP>
-__device__ __forceinline__ void equilibrium_blend(const double (&fin)[NPOP], double (&out)[NPOP], double keep,
-                                                  double scale, double ux, double uz, double T)
+template <bool KEEP, class Load, class Store>
+__device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&store, double keep, double scale,
+                                                       double ux, double uz, double T)
 {
     const double theta = T - 1.0;
     const double q = ux * ux + uz * uz;
@@ -125,51 +164,62 @@ __device__ __forceinline__ void equilibrium_blend(const double (&fin)[NPOP], dou
     const double b0 = b1 + 0.125 * (q * q);
     const double b2 = 0.5 - 0.25 * q;
     // s = e_x A + e_z B with A = r u_x, B = r u_z
-    const double A1 = D2Q37_R * ux, B1 = D2Q37_R * uz;
+    const double A1 = c_lat[0] * ux, B1 = c_lat[0] * uz;
     const double A[4] = {0.0, A1, 2.0 * A1, 3.0 * A1};
     const double B[4] = {0.0, B1, 2.0 * B1, 3.0 * B1};
 
-    double G0[8], G1[8], G2[8], G3[8], G4[8];
     static_for<0, 8>([&](auto S) {
         constexpr int sl = decltype(S)::value;
-        constexpr double c2 = D2Q37_R2 * shell_e2(sl);
-        constexpr double k1 = 0.5 * (c2 - 2.0), k2 = 0.25 * (4.0 - c2), k3 = 0.125 * (c2 * c2 - 8.0 * c2 + 8.0);
-        constexpr double k4 = 0.5 * (c2 - 4.0), k5 = 0.25 * (c2 - 6.0);
-        const double ws = scale * shell_weight(shell_e2(sl));
-        const double g0 = fma(theta, fma(theta, k3, fma(q, k2, k1)), b0);
-        const double g1 = fma(theta, k4, b1);
-        const double g2 = fma(theta, k5, b2);
-        G0[sl] = ws * g0;
-        G1[sl] = ws * g1;
-        G2[sl] = ws * g2;
-        G3[sl] = ws * (1.0 / 6.0);
-        G4[sl] = ws * (1.0 / 24.0);
+        const ShellConst &c = c_shell[sl];
+        const double ws = scale * c.w;
+        const double g0 = ws * fma(theta, fma(theta, c.k3, fma(q, c.k2, c.k1)), b0);
+        const double g1 = ws * fma(theta, c.k4, b1);
+        const double g2 = ws * fma(theta, c.k5, b2);
+        const double g3 = ws * c_lat[2];
+        const double g4 = ws * c_lat[3];
+        static_for<0, NPOP>([&](auto L) {
+            constexpr int l = decltype(L)::value;
+            if constexpr (shell_slot(pop_e2(l)) == sl) {
+                constexpr int ex = pop_ex(l), ez = pop_ez(l);
+                constexpr int ax = ex < 0 ? -ex : ex, az = ez < 0 ? -ez : ez;
+                double s;
+                if constexpr (ex == 0 && ez == 0) s = 0.0;
+                else if constexpr (ez == 0) s = ex > 0 ? A[ax] : -A[ax];
+                else if constexpr (ex == 0) s = ez > 0 ? B[az] : -B[az];
+                else s = (ex > 0 ? A[ax] : -A[ax]) + (ez > 0 ? B[az] : -B[az]);
+                double p;
+                if constexpr (ex == 0 && ez == 0) p = g0;
+                else p = fma(fma(fma(fma(g4, s, g3), s, g2), s, g1), s, g0);
+                if constexpr (KEEP) store(L, fma(keep, load(L), p));
+                else store(L, p);
+            }
+        });
     });
+}
 
-    static_for<0, NPOP>([&](auto L) {
-        constexpr int l = decltype(L)::value;
-        constexpr int ex = pop_ex(l), ez = pop_ez(l), sl = shell_slot(pop_e2(l));
-        constexpr int ax = ex < 0 ? -ex : ex, az = ez < 0 ? -ez : ez;
-        double s;
-        if constexpr (ex == 0 && ez == 0) s = 0.0;
-        else if constexpr (ez == 0) s = ex > 0 ? A[ax] : -A[ax];
-        else if constexpr (ex == 0) s = ez > 0 ? B[az] : -B[az];
-        else s = (ex > 0 ? A[ax] : -A[ax]) + (ez > 0 ? B[az] : -B[az]);
-        double p;
-        if constexpr (ex == 0 && ez == 0) p = G0[sl];
-        else p = fma(fma(fma(fma(G4[sl], s, G3[sl]), s, G2[sl]), s, G1[sl]), s, G0[sl]);
-        if constexpr (KEEP) out[l] = fma(keep, fin[l], p);
-        else out[l] = p;
-    });
+template <bool KEEP>
+__device__ __forceinline__ void equilibrium_blend(const double (&fin)[NPOP], double (&out)[NPOP], double keep,
+                                                  double scale, double ux, double uz, double T)
+{
+    equilibrium_blend_from<KEEP>([&](auto L) { return fin[decltype(L)::value]; },
+                                 [&](auto L, double v) { out[decltype(L)::value] = v; }, keep, scale, ux, uz, T);
 }
 
 // One collision: moments of the post-propagate populations, equilibrium shifted by
 // u' = u + g_vec tau = (u_x, u_z - g tau), T' = T + tau (dt - tau) g^2 / d, BGK relaxation.
 //   omega = dt/tau, gtau = g tau, dT = tau (1 - tau) g^2 / 2.
+// `load` is called twice per population (moments, then relaxation), `store` once.
+template <class Load, class Store>
+__device__ __forceinline__ void collide_from(Load &&load, Store &&store, double omega, double gtau, double dT)
+{
+    const Kinetic k = kinetic_from_raw(raw_moments_from(load));
+    equilibrium_blend_from<true>(load, store, 1.0 - omega, omega * k.rho, k.ux, k.uz - gtau, k.T + dT);
+}
+
 __device__ __forceinline__ void collide_site(double (&f)[NPOP], double omega, double gtau, double dT)
 {
-    const Kinetic k = kinetic_moments(f);
-    equilibrium_blend<true>(f, f, 1.0 - omega, omega * k.rho, k.ux, k.uz - gtau, k.T + dT);
+    collide_from([&](auto L) { return f[decltype(L)::value]; },
+                 [&](auto L, double v) { f[decltype(L)::value] = v; }, omega, gtau, dT);
 }
 
 }  // namespace d2q37

@@ -79,7 +79,8 @@ struct lbm_handle {
     int cur;               // index of the current lattice
     long long steps, launches;
     int variant;
-    int zchunk;            // rows per block of the two-step kernel (multiple of S2_R)
+    int zchunk;            // rows per block of the two-step kernel (multiple of 3; 0 = automatic)
+    int sm_count;
     double *scratch;       // device: Tbar[Lz] | row partials[4 Lz] | results[8] | h_lo[Lx] | h_hi[Lx]
     double *stage[4];      // device staging fields for lbm_run_host (lazy)
     lbm::Layout layout() const { return lbm::Layout{Lx, Lz, pitch, plane}; }
@@ -139,9 +140,9 @@ int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p)
     lbm_handle *h = new (std::nothrow) lbm_handle();
     if (!h) return fail(LBM_ERR_INVALID, "lbm_create: out of host memory");
     h->Lx = Lx; h->Lz = Lz; h->pitch = pitch_of(Lx); h->plane = plane_of(Lx, Lz);
-    h->tau = p->tau; h->g = p->g;
+    h->tau = p->tau; h->g = p->g; h->sm_count = prop.multiProcessorCount;
     h->buf[0] = (double *)p->pop_buf0; h->buf[1] = (double *)p->pop_buf1;
-    h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 192; h->scratch = nullptr;
+    h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 0; h->scratch = nullptr;
     for (auto &s : h->stage) s = nullptr;
     cudaError_t e = cudaMalloc(&h->scratch, sizeof(double) * (5LL * Lz + 8 + 2LL * Lx));
     if (e != cudaSuccess) { delete h; return fail(LBM_ERR_CUDA, "lbm_create: cudaMalloc scratch: %s", cudaGetErrorString(e)); }
@@ -255,35 +256,45 @@ int lbm_step(lbm_t *h, int n, void *stream)
     a.gtau = h->g * h->tau;
     a.dT = 0.5 * h->tau * (1.0 - h->tau) * h->g * h->g;
     lbm::fill_offsets(a);
+    // Variants: 0 = automatic (two steps per launch where the lattice is large enough to fill the GPU with
+    // strips, else one step per launch), 1 = one step, 256x1 blocks, 2 = one step, 128x1 blocks,
+    // 3 = two steps per launch forced.  An odd last step always runs the one-step kernel.
+    using S2 = lbm::Step2Wide;
+    int ZC = h->zchunk;
+    const int strips = (h->Lx + S2::TX - 1) / S2::TX;
+    if (ZC == 0) {  // enough blocks for >= 4 waves over the SMs, chunks of 24..192 rows (warm-up is 6 rows per chunk)
+        const int want_chunks = (4 * h->sm_count + strips - 1) / strips;
+        ZC = (h->Lz + want_chunks - 1) / want_chunks;
+        ZC = (ZC + S2::R - 1) / S2::R * S2::R;
+        if (ZC < 24) ZC = 24;
+        if (ZC > 192) ZC = 192;
+    }
+    const long long blocks2 = (long long)strips * ((h->Lz + ZC - 1) / ZC);
+    const bool fused = h->variant == 3 || (h->variant == 0 && blocks2 >= 2LL * h->sm_count && h->Lx >= 2 * S2::TX);
     int s = 0;
-    if (h->variant == 3) {  // two steps per launch (lbm_step2.cuh); an odd last step falls through
+    if (fused && n >= 2) {
         static bool attr_set = false;
         if (!attr_set) {
-            CUDA_TRY(cudaFuncSetAttribute(lbm::step2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lbm::S2_SMEM));
+            CUDA_TRY(cudaFuncSetAttribute(lbm::step2_kernel<S2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2::SMEM));
             attr_set = true;
         }
-        const int ZC = h->zchunk;
-        dim3 grid((h->Lx + lbm::S2_TX - 1) / lbm::S2_TX, (h->Lz + ZC - 1) / ZC);
+        dim3 grid(strips, (h->Lz + ZC - 1) / ZC);
         for (; s + 2 <= n; s += 2) {
             a.src = h->buf[h->cur];
             a.dst = h->buf[h->cur ^ 1];
-            lbm::step2_kernel<<<grid, lbm::S2_THREADS, lbm::S2_SMEM, st>>>(a, ZC);
+            lbm::step2_kernel<S2><<<grid, S2::THREADS, S2::SMEM, st>>>(a, ZC);
             LAUNCHED(h);
-            h->cur ^= 1;
+            h->cur ^= 1;  // a5: swap prv / nxt, once per two steps
             h->steps += 2;
         }
     }
     for (; s < n; ++s) {
         a.src = h->buf[h->cur];
         a.dst = h->buf[h->cur ^ 1];
-        switch (h->variant) {
-#define LBM_LAUNCH_SITE(TX, TZ)                                                                          \
-    lbm::step_kernel_site<TX, TZ><<<dim3((h->Lx + TX - 1) / TX, (h->Lz + TZ - 1) / TZ), dim3(TX, TZ), 0, st>>>(a)
-        case 1: LBM_LAUNCH_SITE(128, 1); break;
-        case 2: LBM_LAUNCH_SITE(128, 2); break;
-        default: LBM_LAUNCH_SITE(256, 1); break;  // 2 blocks/SM at 128 registers: measured fastest at 4096x8192
-#undef LBM_LAUNCH_SITE
-        }
+        if (h->variant == 2)
+            lbm::step_kernel_site<128, 1><<<dim3((h->Lx + 127) / 128, h->Lz), dim3(128, 1), 0, st>>>(a);
+        else  // 256 threads = 2 blocks/SM at 128 registers: fastest one-step shape at 4096x8192
+            lbm::step_kernel_site<256, 1><<<dim3((h->Lx + 255) / 256, h->Lz), dim3(256, 1), 0, st>>>(a);
         LAUNCHED(h);
         h->cur ^= 1;  // a5: swap prv / nxt
         h->steps++;
@@ -413,7 +424,7 @@ int lbm_kernel_launches(const lbm_t *h, long long *launches)
 int lbm_set_zchunk(lbm_t *h, int rows)
 {
     NEED(h);
-    if (rows < lbm::S2_R || rows % lbm::S2_R) return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be a positive multiple of %d (got %d)", lbm::S2_R, rows);
+    if (rows < 0 || rows % 3) return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be 0 (automatic) or a positive multiple of 3 (got %d)", rows);
     h->zchunk = rows;
     return LBM_OK;
 }

@@ -211,7 +211,7 @@ def test_two_step_kernel_is_bitwise_equal_to_single_steps(pkg, orc, Lx, Lz, zchu
     ux = 0.03 * rng.uniform(-1, 1, (Lz, Lx)); uz = 0.03 * rng.uniform(-1, 1, (Lz, Lx))
     f0 = orc.init_equilibrium(rho, ux, uz, T) * (1 + 0.01 * rng.uniform(-1, 1, (37, Lz, Lx)))
     a, b = pkg.Lattice(Lx, Lz, 0.66, 3e-4), pkg.Lattice(Lx, Lz, 0.66, 3e-4)
-    b.set_variant(3); b.set_zchunk(zchunk)
+    a.set_variant(1); b.set_variant(3); b.set_zchunk(zchunk)
     for lat in (a, b):
         lat.set_populations(torch.from_numpy(f0).cuda())
         lat.step(n)
