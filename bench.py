@@ -28,7 +28,9 @@ BYTES_PER_SITE = 592          # 37 x 8 B read + 37 x 8 B written per site per st
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel at 4096x8192, from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, variant); null for anything not captured.
-NCU_TRAFFIC_BYTES = {("rt_single_4096x8192", 0): 19.814e9}   # profiles/r1_step_kernel_full.md
+# Key: (workload, steps per launch).
+NCU_TRAFFIC_BYTES = {("rt_single_4096x8192", 1): 19.814e9,    # profiles/r1_step_kernel_full.md
+                     ("rt_single_4096x8192", 2): 20.180e9}     # profiles/r1_step2_kernel_full.md
 
 
 def measured_peak():
@@ -195,8 +197,9 @@ def run_ours(args):
     l0 = lat.kernel_launches
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     ev[0].record(stream)
-    lat.step(args.steps)                                     # K launches of the fused step kernel
+    lat.step(args.steps)                                     # K (one-step) or K/2 (two-step kernel) launches
     ev[1].record(stream)
+    step_launches = lat.kernel_launches - l0
     widths = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)   # a6, synchronises
     ev[2].record(stream)
     barrier()
@@ -231,12 +234,24 @@ def run_ours(args):
         return
 
     peak, peak_kind = measured_peak()
-    step_ms = t_steps / args.steps * 1e3
-    achieved = BYTES_PER_SITE * sites / (t_steps / args.steps) / 1e9
-    roofline = {"bound": "hbm", "kernel": "step_kernel (fused propagate+bc+collide)", "achieved": achieved,
-                "peak": peak, "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
+    # Dominant kernel: the step kernel.  Algorithmic bytes per launch = 592 B/site/step x sites x
+    # the steps one launch advances (1: step_kernel_site, 2: step2_kernel, which keeps the intermediate lattice
+    # in shared memory, so its DRAM traffic -- `traffic`, from ncu -- is about half its algorithmic bytes and
+    # `frac` can exceed 1: DESIGN.md section 6).  Launch duration = CUDA-event time of the K steps / launches.
+    spl = args.steps / max(step_launches, 1)
+    launch_ms = t_steps / max(step_launches, 1) * 1e3
+    alg_bytes = BYTES_PER_SITE * sites * spl
+    achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+    traffic = NCU_TRAFFIC_BYTES.get((cfg.name, int(round(spl)))) if abs(spl - round(spl)) < 1e-9 else None
+    roofline = {"bound": "hbm",
+                "kernel": "step2_kernel (two fused propagate+bc+collide steps per launch)" if spl > 1.5
+                else "step_kernel_site (fused propagate+bc+collide)",
+                "achieved": achieved, "peak": peak,
+                "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
                 "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
-                "bytes_per_site": BYTES_PER_SITE, "kernel_ms": step_ms, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, args.variant or 0))}
+                "bytes_per_site_step": BYTES_PER_SITE, "steps_per_launch": spl, "launches": step_launches,
+                "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": launch_ms, "traffic": traffic,
+                "dram_gbs": (traffic / (launch_ms * 1e-3) / 1e9) if traffic else None}
     cpu = None
     if not args.no_cpu_baseline:
         v, cores, sample = oracle_sample_rate(cfg, args.cpu_budget)
