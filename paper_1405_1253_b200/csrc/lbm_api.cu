@@ -14,6 +14,7 @@
 #include "lbm_aux.cuh"
 #include "lbm_step.cuh"
 #include "lbm_step2.cuh"
+#include "lbm_step2s.cuh"
 
 namespace {
 
@@ -270,19 +271,25 @@ int lbm_step(lbm_t *h, int n, void *stream)
         if (ZC > 192) ZC = 192;
     }
     const long long blocks2 = (long long)strips * ((h->Lz + ZC - 1) / ZC);
-    const bool fused = h->variant == 3 || (h->variant == 0 && blocks2 >= 2LL * h->sm_count && h->Lx >= 2 * S2::TX);
+    const bool fused = h->variant == 3 || h->variant == 4 ||
+                       (h->variant == 0 && blocks2 >= 2LL * h->sm_count && h->Lx >= 2 * S2::TX);
+    const bool specialised = h->variant == 4;
+    using S2S = lbm::Step2sWide;
+    static_assert(S2S::TX == S2::TX && S2S::R == S2::R, "both two-step kernels share the strip/chunk selection");
     int s = 0;
     if (fused && n >= 2) {
         static bool attr_set = false;
         if (!attr_set) {
             CUDA_TRY(cudaFuncSetAttribute(lbm::step2_kernel<S2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2::SMEM));
+            CUDA_TRY(cudaFuncSetAttribute(lbm::step2s_kernel<S2S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2S::SMEM));
             attr_set = true;
         }
         dim3 grid(strips, (h->Lz + ZC - 1) / ZC);
         for (; s + 2 <= n; s += 2) {
             a.src = h->buf[h->cur];
             a.dst = h->buf[h->cur ^ 1];
-            lbm::step2_kernel<S2><<<grid, S2::THREADS, S2::SMEM, st>>>(a, ZC);
+            if (specialised) lbm::step2s_kernel<S2S><<<grid, S2S::THREADS, S2S::SMEM, st>>>(a, ZC);
+            else lbm::step2_kernel<S2><<<grid, S2::THREADS, S2::SMEM, st>>>(a, ZC);
             LAUNCHED(h);
             h->cur ^= 1;  // a5: swap prv / nxt, once per two steps
             h->steps += 2;
@@ -432,7 +439,7 @@ int lbm_set_zchunk(lbm_t *h, int rows)
 int lbm_set_variant(lbm_t *h, int variant)
 {
     NEED(h);
-    if (variant < 0 || variant > 3) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
+    if (variant < 0 || variant > 4) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
     h->variant = variant;
     return LBM_OK;
 }

@@ -46,9 +46,10 @@ inline void fill_offsets(StepArgs &a)
 __device__ __forceinline__ double ld_stream(const double *p) { return __ldg(p); }
 __device__ __forceinline__ void st_stream(double *p, double v) { *p = v; }
 
-// Gather the 37 post-propagate populations of site (i, k).  WALL = false: rows 3..Lz-4, no remap.
-template <bool WALL>
-__device__ __forceinline__ void gather_site(const StepArgs &a, int i, int k, double (&f)[NPOP])
+// Pull sources of site (i, k): calls fn(L, p) for l = 0..36 in ascending order, p = address in src of the
+// population that propagation brings to (i, k) as population l.  WALL = false: rows 3..Lz-4, no remap.
+template <bool WALL, class Fn>
+__device__ __forceinline__ void each_source_site(const StepArgs &a, int i, int k, Fn &&fn)
 {
     // periodic x (a1): wrapped source column for each e_x in -3..3
     int col[7];
@@ -78,29 +79,37 @@ __device__ __forceinline__ void gather_site(const StepArgs &a, int i, int k, dou
         constexpr int ex = d2q37::pop_ex(l), ez = d2q37::pop_ez(l);
         int ls = l;
         if (WALL) ls = flip[ez + 3] ? (NPOP - 1 - l) : l;
-        f[l] = ld_stream(a.src + (long long)ls * a.plane + rowoff[ez + 3] + col[ex + 3]);
+        fn(L, a.src + (long long)ls * a.plane + rowoff[ez + 3] + col[ex + 3]);
     });
 }
 
 // Fast path for sites with 3 <= i < Lx-3 and 3 <= k < Lz-3 (no wrap, no wall): every source address is the
 // site's own address plus an offset that depends on kernel arguments only, so the offsets live in uniform
 // registers and each load costs one 64-bit add (the e_x shift is an immediate).
-__device__ __forceinline__ void gather_interior(const StepArgs &a, int i, int k, double (&f)[NPOP])
+template <class Fn>
+__device__ __forceinline__ void each_source_interior(const StepArgs &a, int i, int k, Fn &&fn)
 {
     const char *p = reinterpret_cast<const char *>(a.src + (long long)k * a.pitch + i);
     d2q37::static_for<0, NPOP>([&](auto L) {
         constexpr int l = decltype(L)::value;
-        f[l] = ld_stream(reinterpret_cast<const double *>(p + a.gbyte[l]));
+        fn(L, reinterpret_cast<const double *>(p + a.gbyte[l]));
     });
 }
 
 // dispatch on the site's position: interior / periodic seam / wall rows
-__device__ __forceinline__ void gather_any(const StepArgs &a, int i, int k, double (&f)[NPOP])
+template <class Fn>
+__device__ __forceinline__ void each_source_any(const StepArgs &a, int i, int k, Fn &&fn)
 {
     const bool bulk_z = k >= 3 && k < a.Lz - 3;
-    if (bulk_z && i >= 3 && i < a.Lx - 3) gather_interior(a, i, k, f);
-    else if (bulk_z) gather_site<false>(a, i, k, f);
-    else gather_site<true>(a, i, k, f);
+    if (bulk_z && i >= 3 && i < a.Lx - 3) each_source_interior(a, i, k, fn);
+    else if (bulk_z) each_source_site<false>(a, i, k, fn);
+    else each_source_site<true>(a, i, k, fn);
+}
+
+// Gather the 37 post-propagate populations of site (i, k) into registers.
+__device__ __forceinline__ void gather_any(const StepArgs &a, int i, int k, double (&f)[NPOP])
+{
+    each_source_any(a, i, k, [&](auto L, const double *p) { f[decltype(L)::value] = ld_stream(p); });
 }
 
 __device__ __forceinline__ void scatter_site(const StepArgs &a, int i, int k, const double (&f)[NPOP])
