@@ -1,6 +1,7 @@
 // lbm_api.cu -- the C ABI declared in include/lbm.h: handle, argument checks, kernel launches.
 // Every arithmetic step of the path runs in the kernels of lbm_step.cuh / lbm_aux.cuh; this file only
 // validates, draws the interface perturbation (host, O(Lx)), launches and copies.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -70,6 +71,39 @@ void draw_interface(SplitMix &rng, const lbm_rt_init &ic, int Lx, std::vector<do
     }
 }
 
+// Tensor maps for the TMA loads of the warp-specialised two-step kernel (lbm_step2s.cuh): the lattice copy `buf`
+// as a rank-3 tensor (x: Lx, z: Lz, l: 37) with strides (pitch, plane), box (SP, R, n) for n = 3, 5, 7.
+// cuTensorMapEncodeTiled is fetched through the runtime (no link-time dependency on libcuda).
+bool encode_step2s_maps(const double *buf, int Lx, int Lz, int pitch, long long plane, lbm::Step2sMaps &out)
+{
+    using S = lbm::Step2sWide;
+    typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                 const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn) {
+            cudaGetLastError();
+            return false;
+        }
+        encode = (EncodeFn)fn;
+    }
+    static_assert(sizeof(CUtensorMap) == 128, "Step2sMaps holds three 128-byte tensor maps");
+    for (int i = 0; i < 3; ++i) {
+        const cuuint64_t dims[3] = {(cuuint64_t)Lx, (cuuint64_t)Lz, (cuuint64_t)LBM_NPOP};
+        const cuuint64_t strides[2] = {(cuuint64_t)pitch * 8, (cuuint64_t)plane * 8};
+        const cuuint32_t box[3] = {(cuuint32_t)S::SP, (cuuint32_t)S::R, (cuuint32_t)(3 + 2 * i)};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        if (encode((CUtensorMap *)out.m[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)buf, dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return false;
+    }
+    return true;
+}
+
 }  // namespace
 
 struct lbm_handle {
@@ -82,6 +116,8 @@ struct lbm_handle {
     int variant;
     int zchunk;            // rows per block of the two-step kernel (multiple of 3; 0 = automatic)
     int sm_count;
+    bool tma_ok;              // tensor maps of both lattice copies encoded (two-step kernel, variant 4)
+    lbm::Step2sMaps maps[2];
     double *scratch;       // device: Tbar[Lz] | row partials[4 Lz] | results[8] | h_lo[Lx] | h_hi[Lx]
     double *stage[4];      // device staging fields for lbm_run_host (lazy)
     lbm::Layout layout() const { return lbm::Layout{Lx, Lz, pitch, plane}; }
@@ -144,6 +180,8 @@ int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p)
     h->tau = p->tau; h->g = p->g; h->sm_count = prop.multiProcessorCount;
     h->buf[0] = (double *)p->pop_buf0; h->buf[1] = (double *)p->pop_buf1;
     h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 0; h->scratch = nullptr;
+    h->tma_ok = encode_step2s_maps(h->buf[0], Lx, Lz, h->pitch, h->plane, h->maps[0]) &&
+                encode_step2s_maps(h->buf[1], Lx, Lz, h->pitch, h->plane, h->maps[1]);
     for (auto &s : h->stage) s = nullptr;
     cudaError_t e = cudaMalloc(&h->scratch, sizeof(double) * (5LL * Lz + 8 + 2LL * Lx));
     if (e != cudaSuccess) { delete h; return fail(LBM_ERR_CUDA, "lbm_create: cudaMalloc scratch: %s", cudaGetErrorString(e)); }
@@ -266,7 +304,7 @@ int lbm_step(lbm_t *h, int n, void *stream)
     if (ZC == 0) {  // enough blocks for >= 4 waves over the SMs, chunks of 24..192 rows (warm-up is 6 rows per chunk)
         const int want_chunks = (4 * h->sm_count + strips - 1) / strips;
         ZC = (h->Lz + want_chunks - 1) / want_chunks;
-        ZC = (ZC + S2::R - 1) / S2::R * S2::R;
+        ZC = (ZC + 5) / 6 * 6;   // whole passes of either two-step kernel (3 or 2 rows)
         if (ZC < 24) ZC = 24;
         if (ZC > 192) ZC = 192;
     }
@@ -274,8 +312,9 @@ int lbm_step(lbm_t *h, int n, void *stream)
     const bool fused = h->variant == 3 || h->variant == 4 ||
                        (h->variant == 0 && blocks2 >= 2LL * h->sm_count && h->Lx >= 2 * S2::TX);
     const bool specialised = h->variant == 4;
+    if (specialised && !h->tma_ok) return fail(LBM_ERR_CUDA, "lbm_step: variant 4 needs tensor maps (cuTensorMapEncodeTiled failed)");
     using S2S = lbm::Step2sWide;
-    static_assert(S2S::TX == S2::TX && S2S::R == S2::R, "both two-step kernels share the strip/chunk selection");
+    static_assert(S2S::TX == S2::TX, "both two-step kernels share the strip/chunk selection");
     int s = 0;
     if (fused && n >= 2) {
         static bool attr_set = false;
@@ -288,7 +327,7 @@ int lbm_step(lbm_t *h, int n, void *stream)
         for (; s + 2 <= n; s += 2) {
             a.src = h->buf[h->cur];
             a.dst = h->buf[h->cur ^ 1];
-            if (specialised) lbm::step2s_kernel<S2S><<<grid, S2S::THREADS, S2S::SMEM, st>>>(a, ZC);
+            if (specialised) lbm::step2s_kernel<S2S><<<grid, S2S::THREADS, S2S::SMEM, st>>>(a, h->maps[h->cur], ZC);
             else lbm::step2_kernel<S2><<<grid, S2::THREADS, S2::SMEM, st>>>(a, ZC);
             LAUNCHED(h);
             h->cur ^= 1;  // a5: swap prv / nxt, once per two steps
