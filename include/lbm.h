@@ -139,7 +139,7 @@ int lbm_kernel_launches(const lbm_t *h, long long *launches);       /* kernels l
 /* Step-kernel variant: 0 automatic (default), 1 one step per launch (256-thread blocks), 2 one step (128),
  * 3 two steps per launch forced (lbm_step2.cuh).  All give bit-identical results. */
 int lbm_set_variant(lbm_t *h, int variant);
-int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel; a multiple of 3, or 0 = automatic */
+int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel, or 0 = automatic */
 /* D2Q37 tables as the library uses them (host outputs, any may be NULL): e_x[37], e_z[37], w[37], r. */
 int lbm_tables(int *ex, int *ez, double *w, double *r);
 const char *lbm_last_error(void);

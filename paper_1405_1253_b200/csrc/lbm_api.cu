@@ -14,7 +14,6 @@
 #include "../../include/lbm.h"
 #include "lbm_aux.cuh"
 #include "lbm_step.cuh"
-#include "lbm_step2.cuh"
 #include "lbm_step2s.cuh"
 
 namespace {
@@ -116,7 +115,7 @@ struct lbm_handle {
     int variant;
     int zchunk;            // rows per block of the two-step kernel (multiple of 3; 0 = automatic)
     int sm_count;
-    bool tma_ok;              // tensor maps of both lattice copies encoded (two-step kernel, variant 4)
+    bool tma_ok;              // tensor maps of both lattice copies encoded (two-step kernel)
     lbm::Step2sMaps maps[2];
     double *scratch;       // device: Tbar[Lz] | row partials[4 Lz] | results[8] | h_lo[Lx] | h_hi[Lx]
     double *stage[4];      // device staging fields for lbm_run_host (lazy)
@@ -298,37 +297,33 @@ int lbm_step(lbm_t *h, int n, void *stream)
     // Variants: 0 = automatic (two steps per launch where the lattice is large enough to fill the GPU with
     // strips, else one step per launch), 1 = one step, 256x1 blocks, 2 = one step, 128x1 blocks,
     // 3 = two steps per launch forced.  An odd last step always runs the one-step kernel.
-    using S2 = lbm::Step2Wide;
+    using S2 = lbm::Step2sWide;
     int ZC = h->zchunk;
     const int strips = (h->Lx + S2::TX - 1) / S2::TX;
     if (ZC == 0) {  // enough blocks for >= 4 waves over the SMs, chunks of 24..192 rows (warm-up is 6 rows per chunk)
         const int want_chunks = (4 * h->sm_count + strips - 1) / strips;
         ZC = (h->Lz + want_chunks - 1) / want_chunks;
-        ZC = (ZC + 5) / 6 * 6;   // whole passes of either two-step kernel (3 or 2 rows)
+        ZC = (ZC + 5) / 6 * 6;   // whole passes for R = 2 or 3 rows
         if (ZC < 24) ZC = 24;
         if (ZC > 192) ZC = 192;
     }
     const long long blocks2 = (long long)strips * ((h->Lz + ZC - 1) / ZC);
-    const bool fused = h->variant == 3 || h->variant == 4 ||
-                       (h->variant == 0 && blocks2 >= 2LL * h->sm_count && h->Lx >= 2 * S2::TX);
-    const bool specialised = h->variant == 4;
-    if (specialised && !h->tma_ok) return fail(LBM_ERR_CUDA, "lbm_step: variant 4 needs tensor maps (cuTensorMapEncodeTiled failed)");
-    using S2S = lbm::Step2sWide;
-    static_assert(S2S::TX == S2::TX, "both two-step kernels share the strip/chunk selection");
+    const bool fused = h->variant == 3 ||
+                       (h->variant == 0 && h->tma_ok && blocks2 >= 2LL * h->sm_count && h->Lx >= 2 * S2::TX);
+    if (h->variant == 3 && !h->tma_ok)
+        return fail(LBM_ERR_CUDA, "lbm_step: the two-step kernel needs tensor maps (cuTensorMapEncodeTiled failed)");
     int s = 0;
     if (fused && n >= 2) {
         static bool attr_set = false;
         if (!attr_set) {
-            CUDA_TRY(cudaFuncSetAttribute(lbm::step2_kernel<S2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2::SMEM));
-            CUDA_TRY(cudaFuncSetAttribute(lbm::step2s_kernel<S2S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2S::SMEM));
+            CUDA_TRY(cudaFuncSetAttribute(lbm::step2s_kernel<S2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2::SMEM));
             attr_set = true;
         }
         dim3 grid(strips, (h->Lz + ZC - 1) / ZC);
         for (; s + 2 <= n; s += 2) {
             a.src = h->buf[h->cur];
             a.dst = h->buf[h->cur ^ 1];
-            if (specialised) lbm::step2s_kernel<S2S><<<grid, S2S::THREADS, S2S::SMEM, st>>>(a, h->maps[h->cur], ZC);
-            else lbm::step2_kernel<S2><<<grid, S2::THREADS, S2::SMEM, st>>>(a, ZC);
+            lbm::step2s_kernel<S2><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], ZC);
             LAUNCHED(h);
             h->cur ^= 1;  // a5: swap prv / nxt, once per two steps
             h->steps += 2;
@@ -470,7 +465,7 @@ int lbm_kernel_launches(const lbm_t *h, long long *launches)
 int lbm_set_zchunk(lbm_t *h, int rows)
 {
     NEED(h);
-    if (rows < 0 || rows % 3) return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be 0 (automatic) or a positive multiple of 3 (got %d)", rows);
+    if (rows < 0) return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be 0 (automatic) or positive (got %d)", rows);
     h->zchunk = rows;
     return LBM_OK;
 }
@@ -478,7 +473,7 @@ int lbm_set_zchunk(lbm_t *h, int rows)
 int lbm_set_variant(lbm_t *h, int variant)
 {
     NEED(h);
-    if (variant < 0 || variant > 4) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
+    if (variant < 0 || variant > 3) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
     h->variant = variant;
     return LBM_OK;
 }

@@ -1,40 +1,72 @@
-// lbm_step2s.cuh -- two time steps per launch, WARP-SPECIALISED (producer / consumer) version of lbm_step2.cuh.
+// lbm_step2s.cuh -- TWO time steps per launch (temporal blocking): propagate+bc+collide, twice, with
+// the intermediate lattice f1 = step(f0) kept in shared memory, so that HBM sees ~296 B read + 296 B written per
+// site per TWO steps instead of per step.  Warp-specialised: loader / producer / consumer warps.
 //
-// Same decomposition as step2_kernel (a block owns a strip of TX output columns and marches up ZC rows, the
-// intermediate lattice f1 = step(f0) lives in a shared-memory ring, halo columns are recomputed), but
-//   * the first step (pass A: global gather -> collide -> ring) and the second step (pass B: ring gather ->
-//     collide -> global store) run on DIFFERENT warps, so one side's memory latency overlaps the other side's
-//     FP64 arithmetic instead of all warps marching in phase;
-//   * pass A's inputs are prefetched a pass ahead into a shared-memory stage by a LOADER warp with TMA tensor box
-//     loads (seven per pass) instead of into 74 registers per thread, so 14 warps of 128 registers fit where 8 of
-//     253 did;
-//   * the ring keeps, per population, only the rows that can still be read: population l of intermediate row q is
-//     read by the output row q + e_lz, so its ring has depth R + 3 + e_lz rows (R .. R + 6) instead of R + 6 for
-//     all: 222 instead of 333 row-populations at R = 3, which is what makes room for the stage;
-//   * the bottom wall is realised by three GHOST ring rows (rows -3..-1 hold the velocity-reversed copy of rows
-//     2..0, written by the producer of those rows; the "ghost row" picture of DESIGN.md reading 9), so pass B's
-//     gather is uniform there; at the top wall the mirror rows are still resident and pass B remaps indices.
+// A block owns a strip of TX output columns and marches up a chunk of ZC rows, R rows per pass.
+//   loader (1 warp)   the gather part of the first step: seven TMA tensor box loads per pass (one per e_z) bring the
+//                     source rows of the pass into a shared-memory STAGE, NST passes ahead;
+//   producers         one thread per site of the R x (TX+6) intermediate slab (three halo columns per side are
+//                     recomputed, not exchanged): read the 37 populations from the stage with the e_x shift, collide
+//                     in registers, store f1 into the RING;
+//   consumers         one thread per output site: gather the 37 populations from ring rows k-3..k+3, collide, write
+//                     f2 to global memory with aligned full-line stores.
+// Ring: population l of intermediate row q is read only by output row q + e_lz, so its ring keeps R + 3 + e_lz rows
+// (R .. R+6) instead of R+6 for all -- 37 (R+3) row-populations instead of 37 (R+6), which is what makes room for
+// the stage.  Bottom wall (a3): three GHOST ring rows -3..-1 hold the velocity-reversed copy of rows 2..0 (the ghost
+// row picture of DESIGN.md reading 9), written by the producers of those rows, so the consumers' gather is uniform
+// there; at the top wall the mirror rows are still resident and the consumers remap indices.  Sites whose first-step
+// sources wrap (seam strips, a1) or reflect (wall rows) are gathered from global memory by their producer thread;
+// the TMA unit zero-fills those parts of the boxes and they are never read.
 // Arithmetic is raw_moments / kinetic_from_raw / equilibrium_blend of d2q37.cuh, i.e. exactly collide_site():
 // results are bit-identical to two launches of the one-step kernel (tested).
 //
-// Hand-offs (mbarriers, arrive early / wait late).  Producer pass j writes intermediate rows q in [jR, jR+R)
-// (q = row - z0 + 3); consumer pass i reads rows iR .. iR+R+5.
-//   FULL : consumer pass i waits for producer passes <= i + LEAD,  LEAD = 1 + 5/R (phase i of the barrier:
-//          producers start arriving at pass LEAD, each thread's arrival covers all its earlier passes)
-//   EMPTY: producer pass j overwrites slots last read by consumer pass j - LAG, LAG = ceil(7/R), and waits for it.
+// Hand-offs are mbarriers.  Producer pass j writes intermediate rows q in [jR, jR+R) (q = row - z0 + 3); consumer
+// pass i reads rows iR .. iR+R+5.
+//   FULL  (producers -> consumers): consumer pass i waits for producer passes <= i + LEAD, LEAD = 1 + 5/R;
+//   EMPTY (consumers -> producers): producer pass j overwrites slots last read by consumer pass j - LAG,
+//         LAG = ceil(7/R) + SL (SL = optional extra ring depth in passes);
+//   STAGE_FULL / STAGE_EMPTY (loader <-> producers), one pair per stage buffer; the TMA loads complete STAGE_FULL.
+// A buffer (stage or ring rows) is released only after its values have been CONSUMED by arithmetic, not merely
+// loaded: mbarrier.arrive does not wait for shared-memory loads in flight, and a TMA write that the release allows
+// was observed to overtake them (profiles/r1_two_step.md).
+//
+// Measured and dropped on the way (profiles/r1_two_step.md): all warps doing both steps in phase with the first
+// step's inputs prefetched into 74 registers (8 warps of 253 registers, 15.0 GLUPS); per-thread 8-byte cp.async into
+// the stage (~20 cycles of L1TEX per warp instruction, and L1TEX returns in order, so the issuing warp's next
+// local/global load waits for DRAM); one 1-D bulk copy per row and population (the TMA unit issues one copy per
+// ~63 cycles whatever its size).
 #pragma once
 #include "lbm_step.cuh"
-#include "lbm_step2.cuh"   // mbar_* helpers
 
 namespace lbm {
 
-template <int TX_, int R_, int NST_>
+// split-phase barriers on mbarriers in shared memory
+__device__ __forceinline__ void mbar_init(unsigned bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+
+template <int TX_, int R_, int NST_, int SL_>
 struct Step2sShape {
     static constexpr int TX = TX_;                      // output columns per strip (multiple of 32)
     static constexpr int W1 = TX_ + 6;                  // intermediate columns per strip
     static constexpr int CP = TX_ + 8;                  // ring row pitch (doubles)
     static constexpr int R = R_;                        // rows per pass
     static constexpr int NST = NST_;                    // stage buffers (passes of input in flight)
+    static constexpr int SL = SL_;                      // ring slack: passes the producers may run ahead of the consumers
+    static constexpr int NRB = SL_ + 1;                 // FULL / EMPTY barriers (pass i uses barrier i mod NRB)
     static constexpr int NA = (R_ * (TX_ + 6) + 31) / 32;   // producer warps (one thread per intermediate site)
     static constexpr int NB = R_ * TX_ / 32;                // consumer warps (one thread per output site)
     static constexpr int NAT = NA * 32, NBT = NB * 32;
@@ -42,8 +74,8 @@ struct Step2sShape {
     static constexpr int SP = TX_ + 16;                     // stage row pitch = source span x0-8 .. x0+TX+7 (doubles)
     static constexpr int THREADS = NAT + NBT + NLT;
     static constexpr int LEAD = 1 + 5 / R_;
-    static constexpr int LAG = (7 + R_ - 1) / R_;
-    __host__ __device__ static constexpr int depth(int ez) { return R_ + 3 + ez; }
+    static constexpr int LAG = (7 + R_ - 1) / R_ + SL_;
+    __host__ __device__ static constexpr int depth(int ez) { return R_ + 3 + ez + SL_ * R_; }
     // first ring row (in units of rows of CP doubles) of population l: populations are stacked, each with its depth
     __host__ __device__ static constexpr int row_base(int l)
     {
@@ -52,15 +84,16 @@ struct Step2sShape {
         return s;
     }
     static constexpr int RING_ROWS = row_base(NPOP);
-    static constexpr size_t RING_DOUBLES = (size_t)RING_ROWS * CP;
+    static constexpr size_t RING_DOUBLES = ((size_t)RING_ROWS * CP + 15) / 16 * 16;   // stage starts on a 128-byte line
     static constexpr size_t STAGE_DOUBLES = (size_t)NPOP * R_ * SP;   // per buffer
     static constexpr size_t SMEM = sizeof(double) * (RING_DOUBLES + NST_ * STAGE_DOUBLES);
     static_assert(TX_ % 32 == 0, "a consumer warp covers 32 columns of one row");
     static_assert(R_ >= 2 && NST_ >= 1 && NST_ <= 4, "shape");
     static_assert((R_ * SP * 8) % 128 == 0 && (RING_DOUBLES * 8) % 128 == 0, "TMA box destinations are 128-byte aligned");
-    static_assert(LAG < LEAD + 3, "producer may run at most one FULL phase ahead of the consumer's wait");
 };
-using Step2sWide = Step2sShape<64, 3, 1>;   // 7 producer + 6 consumer + 1 loader warps; ring 127 872 B + stage 71 040 B
+// Measured at 4096x8192 (profiles/r1_two_step.md): <64,2,2,0> 15.5 GLUPS; <64,3,1,0> 14.7 (no room for a second stage
+// buffer: the producers wait for the TMA round trip); <64,2,1,1> 14.2 (ring slack instead of the second buffer).
+using Step2sWide = Step2sShape<64, 2, 2, 0>;   // 5 producer + 4 consumer + 1 loader warps; ring 106 560 B + 2 x 47 360 B stage
 
 // Tensor maps of the source lattice (host-encoded, lbm_api.cu): rank 3 (x: Lx, z: Lz, l: 37), strides
 // (pitch, plane) doubles, box (SP, R, n) for n = 3, 5, 7 -- the populations with the same e_z are consecutive in l.
@@ -118,6 +151,8 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
     const bool xwrap = c - 3 < 0 || c + 3 >= a.Lx;      // a source column wraps: the site is gathered from global memory
     int ac = c % a.Lx;
     if (ac < 0) ac += a.Lx;
+    const int Lz = a.Lz;                                // kernel arguments into registers once (see the consumer)
+    const double omega = a.omega, gtau = a.gtau, dT = a.dT;
 
     const int npass = NP + S::LEAD;
     int b = 0;
@@ -128,18 +163,30 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
         double f[NPOP];
         // sites whose sources wrap (seam strips) or reflect (wall rows, a3) bypass the stage; their loads are issued
         // before the wait so that they overlap it
-        const bool gl = v && (xwrap || row < 3 || row >= a.Lz - 3);
-        if (gl) gather_any(a, ac, row, f);
+        const bool gl = v && (xwrap || row < 3 || row >= Lz - 3);
+        if (gl) each_source_any(a, ac, row, [&](auto L, const double *p) { f[decltype(L)::value] = __ldcg(p); });
         mbar_wait(bar_sfull + 8 * b, use & 1u);
         const double *sb = sp + b * S::STAGE_DOUBLES;
         if (v && !gl) d2q37::static_for<0, NPOP>([&](auto L) {
             constexpr int l = decltype(L)::value;
             f[l] = sb[l * S::R * S::SP - d2q37::pop_ex(l)];
         });
-        mbar_arrive(bar_sempty + 8 * b);                // values are in registers: the buffer may be refilled
+        // The buffer is released only after the moments have CONSUMED the 37 values (not merely after the loads were
+        // issued): mbarrier.arrive does not wait for shared-memory loads in flight, and the TMA write that the
+        // release allows was seen to overtake them (L2-resident source rows, loads held back behind the global
+        // gathers of the same warp) -- a one-in-10^5-blocks error, profiles/r1_two_step.md.
+        d2q37::RawMoments m;
+        if (v) {
+            m = d2q37::raw_moments(f);
+            asm volatile("" : "+d"(m.m0), "+d"(m.jx), "+d"(m.jz), "+d"(m.m2));
+        }
+        mbar_arrive(bar_sempty + 8 * b);
         if (++b == S::NST) { b = 0; ++use; }
-        if (v) d2q37::collide_site(f, a.omega, a.gtau, a.dT);
-        if (j >= S::LAG) mbar_wait(bar_empty, (unsigned)(j - S::LAG) & 1u);
+        if (v) {
+            const d2q37::Kinetic kin = d2q37::kinetic_from_raw(m);
+            d2q37::equilibrium_blend<true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
+        }
+        if (j >= S::LAG) mbar_wait(bar_empty + 8 * ((j - S::LAG) % S::NRB), (unsigned)((j - S::LAG) / S::NRB) & 1u);
         if (v) {
             double *rp = ring + aj;
             const int qrow = j * S::R + ar;             // intermediate row index within the chunk, q = row - z0 + 3
@@ -171,7 +218,7 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
                 });
             }
         }
-        if (j >= S::LEAD) mbar_arrive(bar_full);        // FULL phase i = "passes <= i + LEAD are in the ring"
+        if (j >= S::LEAD) mbar_arrive(bar_full + 8 * ((j - S::LEAD) % S::NRB));   // FULL of consumer pass i = j - LEAD: "passes <= i + LEAD are in the ring"
     }
 }
 
@@ -183,14 +230,21 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
     const int br = bt / S::TX, bj = bt - br * S::TX;
     const bool b_lane = bj < ncols;
     const double *q = ring + bj + 3;
+    // kernel arguments into registers once: `a` is reached through a pointer here (non-inlined role), and every
+    // global store would otherwise force its fields to be re-loaded
+    const int Lz = a.Lz;
+    const double omega = a.omega, gtau = a.gtau, dT = a.dT;
+    const long long plane = a.plane;
+    double *const out = a.dst + (long long)(z0 + br) * a.pitch + x0 + bj;    // this thread's site of pass 0, population 0
+    const long long pass_stride = (long long)S::R * a.pitch;
 
     for (int i = 0; i < NP; ++i) {
         const int k = z0 + i * S::R + br;
         const bool bv = b_lane && k < zend;
-        mbar_wait(bar_full, (unsigned)i & 1u);
+        mbar_wait(bar_full + 8 * (i % S::NRB), (unsigned)(i / S::NRB) & 1u);
         double f[NPOP];
         if (bv) {
-            if (k < a.Lz - 3) {                         // uniform gather (bottom wall included: ghost rows)
+            if (k < Lz - 3) {                           // uniform gather (bottom wall included: ghost rows)
                 // ring slot (in doubles) of the SOURCE row k - e_z, per e_z: q = k - e_z - z0 + 3
                 int slot[7];
 #pragma unroll
@@ -205,8 +259,8 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
 #pragma unroll
                 for (int e = -3; e <= 3; ++e) {
                     int ks = k - e;
-                    const bool fl = ks >= a.Lz;
-                    if (fl) ks = 2 * a.Lz - 1 - ks;
+                    const bool fl = ks >= Lz;
+                    if (fl) ks = 2 * Lz - 1 - ks;
                     off[e + 3] = ((ks - z0 + 3) % (fl ? S::depth(-e) : S::depth(e))) * S::CP;
                     flip[e + 3] = fl;
                 }
@@ -218,10 +272,20 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
                 });
             }
         }
-        mbar_arrive(bar_empty);
+        d2q37::RawMoments m;                            // release the ring rows after the values were consumed (see the producer)
         if (bv) {
-            d2q37::collide_site(f, a.omega, a.gtau, a.dT);
-            scatter_site(a, x0 + bj, k, f);
+            m = d2q37::raw_moments(f);
+            asm volatile("" : "+d"(m.m0), "+d"(m.jx), "+d"(m.jz), "+d"(m.m2));
+        }
+        mbar_arrive(bar_empty + 8 * (i % S::NRB));
+        if (bv) {
+            const d2q37::Kinetic kin = d2q37::kinetic_from_raw(m);
+            d2q37::equilibrium_blend<true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
+            double *p = out + i * pass_stride;          // 37 aligned stores, full 128-byte lines per warp
+            d2q37::static_for<0, NPOP>([&](auto L) {
+                constexpr int l = decltype(L)::value;
+                st_stream(p + l * plane, f[l]);
+            });
         }
     }
 }
@@ -230,19 +294,19 @@ template <class S>
 __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_constant__ StepArgs a, const __grid_constant__ Step2sMaps maps, const int ZC)
 {
     extern __shared__ __align__(128) double smem2s[];    // ring [RING_ROWS][CP] | stage [NST][NPOP][R][SP]
-    __shared__ unsigned long long bars[2 + 2 * S::NST];
+    __shared__ unsigned long long bars[2 * S::NRB + 2 * S::NST];
     const int tid = threadIdx.x;
     const int x0 = blockIdx.x * S::TX, z0 = blockIdx.y * ZC;
     const int ncols = min(S::TX, a.Lx - x0);            // output columns of this strip
     const int zend = min(a.Lz, z0 + ZC);                // output rows [z0, zend)
     const int rlast = min(a.Lz, zend + 3);              // intermediate rows [max(0, z0-3), rlast)
     const int NP = (zend - z0 + S::R - 1) / S::R;       // consumer passes
-    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(&bars[0]);     // ring rows written (producers -> consumers)
-    const unsigned bar_empty = (unsigned)__cvta_generic_to_shared(&bars[1]);    // ring rows read    (consumers -> producers)
-    const unsigned bar_sfull = (unsigned)__cvta_generic_to_shared(&bars[2]);    // [NST] stage buffer filled (loaders -> producers)
+    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(&bars[0]);     // [NRB] ring rows written (producers -> consumers)
+    const unsigned bar_empty = bar_full + 8 * S::NRB;                           // [NRB] ring rows read    (consumers -> producers)
+    const unsigned bar_sfull = bar_empty + 8 * S::NRB;                          // [NST] stage buffer filled (loaders -> producers)
     const unsigned bar_sempty = bar_sfull + 8 * S::NST;                         // [NST] stage buffer read   (producers -> loaders)
     if (tid == 0) {
-        mbar_init(bar_full, S::NAT); mbar_init(bar_empty, S::NBT);
+        for (int b = 0; b < S::NRB; ++b) { mbar_init(bar_full + 8 * b, S::NAT); mbar_init(bar_empty + 8 * b, S::NBT); }
         for (int b = 0; b < S::NST; ++b) { mbar_init(bar_sfull + 8 * b, 1); mbar_init(bar_sempty + 8 * b, S::NAT); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }

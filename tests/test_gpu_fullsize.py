@@ -93,3 +93,23 @@ def test_largest_sweep_lattice_offsets_beyond_32_bits(pkg, orc):
     after = lat.get_populations()
     _check_windows(orc, before, after, Lx, Lz, si.SWEEP_TAU, si.SWEEP_G, 1e-13)
     lat.close()
+
+
+@pytest.mark.gpu
+def test_two_step_kernel_back_to_back_launches_stay_bitwise_equal(pkg):
+    """Regression for a shared-memory hand-off race of the two-step kernel that only showed with many launches back
+    to back on a lattice of >= 1024 x 2048 (a stage buffer released before its loads had completed was overwritten
+    by the next TMA load when the source rows were L2-resident; about one block in 1e5): 200 steps in one call,
+    default (two-step) kernel against the one-step kernel, every population of every site, bit for bit."""
+    import torch
+    Lx, Lz = 1024, 2048
+    fields = si.sweep_fields_torch(Lx, Lz, si.DEFAULT_SEED, "cuda")
+    a, b = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G), pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G)
+    a.set_variant(1)
+    l0 = b.kernel_launches
+    for lat in (a, b):
+        lat.init_equilibrium(*fields)
+        lat.step(200)
+    assert b.kernel_launches - l0 == 1 + 100          # init + 100 two-step launches: the default path is the fused one
+    assert torch.equal(a.get_populations(), b.get_populations())
+    a.close(); b.close()

@@ -49,7 +49,7 @@ def test_config1_init_matches_oracle(pkg, orc):
     lat.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_config1_100_steps_population_parity(pkg, orc, variant):
     """BASELINE.json configs[0]: 64x128 double-front RT, 100 steps, every population of every site."""
     cfg = si.rt_config(1)
@@ -199,11 +199,12 @@ def test_step_is_cuda_graph_capturable(pkg):
 
 
 @pytest.mark.parametrize("Lx,Lz,zchunk,n", [(7, 6, 3, 4), (33, 9, 3, 5), (64, 128, 192, 6), (130, 70, 9, 7),
-                                            (257, 40, 15, 4), (520, 18, 126, 2), (70, 64, 12, 10), (191, 37, 21, 3)])
-@pytest.mark.parametrize("fused_variant", [3, 4])
+                                            (257, 40, 15, 4), (520, 18, 126, 2), (70, 64, 12, 10), (191, 37, 21, 3),
+                                            (130, 70, 7, 4), (200, 50, 10, 6), (128, 31, 5, 2)])
+@pytest.mark.parametrize("fused_variant", [3])
 def test_two_step_kernel_is_bitwise_equal_to_single_steps(pkg, orc, Lx, Lz, zchunk, n, fused_variant):
-    """Variants 3 and 4 fuse two time steps per launch through shared memory (lbm_step2.cuh; lbm_step2s.cuh is the
-    warp-specialised version with per-population ring depths and ghost rows).  They use the same
+    """Variant 3 fuses two time steps per launch through shared memory (lbm_step2s.cuh: TMA loader, producer and
+    consumer warps, per-population ring depths, ghost rows).  It uses the same
     collide arithmetic, so the result must be bit-identical to n single steps (odd n: last step unfused) --
     for ragged strips, chunks that do not divide Lz, lattices made only of wall rows -- and within the oracle
     tolerance."""
