@@ -149,11 +149,20 @@ __device__ __forceinline__ Kinetic kinetic_moments(const double (&f)[NPOP]) { re
 //   g0 = 1 - q/2 + q^2/8 + theta [ (c2-2)/2 + q (4-c2)/4 ] + theta^2 (c2^2 - 8 c2 + 8)/8
 //   g1 = 1 - q/2 + theta (c2-4)/2
 //   g2 = 1/2 - q/4 + theta (c2-6)/4
-// so each population costs one Horner evaluation (4 FMA) plus the relaxation FMA.  Shells are the outer
-// loop: only one shell's five coefficients are live at a time (register pressure), and every population's
-// value is the same expression whichever order the populations are visited in.
+// Opposite populations l and 36 - l share the shell and have s of opposite sign, so the quartic is evaluated once
+// per PAIR as an even and an odd part in t = s^2,
+//   E = g0 + t (g2 + t/24),  O = s (g1 + t/6),   f_eq(l) = E + O,  f_eq(36-l) = E - O
+// (10 FP64 operations per pair including s and the two relaxations, against 12 for two Horner evaluations, and
+// two independent dependency chains per pair instead of one per population).  The 18 pairs are processed in four
+// batches of shells, stage by stage across the pairs of a batch, so that 8-12 independent chains are in flight per
+// thread and only one batch's coefficients are live at a time (register pressure).
 //   collision (rhs of eq. 5): keep = 1 - 1/tau, scale = rho/tau, load = post-propagate f
 //   plain equilibrium:                      keep = 0,         scale = rho
+__host__ __device__ constexpr int shell_batch(int slot)  // shells {0,1,2} {3,5,6} {4} {7}: 4-6 pairs per batch
+{
+    return slot <= 2 ? 0 : slot == 4 ? 2 : slot == 7 ? 3 : 1;
+}
+
 template <bool KEEP, class Load, class Store>
 __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&store, double keep, double scale,
                                                        double ux, double uz, double T)
@@ -167,31 +176,67 @@ __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&stor
     const double A1 = c_lat[0] * ux, B1 = c_lat[0] * uz;
     const double A[4] = {0.0, A1, 2.0 * A1, 3.0 * A1};
     const double B[4] = {0.0, B1, 2.0 * B1, 3.0 * B1};
+    constexpr int REST = NPOP / 2;               // l = 18, e = (0, 0)
 
-    static_for<0, 8>([&](auto S) {
-        constexpr int sl = decltype(S)::value;
-        const ShellConst &c = c_shell[sl];
-        const double ws = scale * c.w;
-        const double g0 = ws * fma(theta, fma(theta, c.k3, fma(q, c.k2, c.k1)), b0);
-        const double g1 = ws * fma(theta, c.k4, b1);
-        const double g2 = ws * fma(theta, c.k5, b2);
-        const double g3 = ws * c_lat[2];
-        const double g4 = ws * c_lat[3];
-        static_for<0, NPOP>([&](auto L) {
+    static_for<0, 4>([&](auto BI) {
+        constexpr int bi = decltype(BI)::value;
+        double g0[8], g1[8], g2[8], g3[8], g4[8];                    // per shell of the batch (others never touched)
+        static_for<0, 8>([&](auto S) {
+            constexpr int sl = decltype(S)::value;
+            if constexpr (shell_batch(sl) == bi) {
+                const ShellConst &c = c_shell[sl];
+                const double ws = scale * c.w;
+                g0[sl] = ws * fma(theta, fma(theta, c.k3, fma(q, c.k2, c.k1)), b0);
+                g1[sl] = ws * fma(theta, c.k4, b1);
+                g2[sl] = ws * fma(theta, c.k5, b2);
+                g3[sl] = ws * c_lat[2];
+                g4[sl] = ws * c_lat[3];
+            }
+        });
+        if constexpr (bi == 0) {
+            if constexpr (KEEP) store(std::integral_constant<int, REST>{}, fma(keep, load(std::integral_constant<int, REST>{}), g0[0]));
+            else store(std::integral_constant<int, REST>{}, g0[0]);
+        }
+        // pairs (l, 36 - l), l = 19..36, of the shells of this batch: stage by stage
+        double s[NPOP], t[NPOP], ev[NPOP], od[NPOP];
+        static_for<REST + 1, NPOP>([&](auto L) {
             constexpr int l = decltype(L)::value;
-            if constexpr (shell_slot(pop_e2(l)) == sl) {
+            if constexpr (shell_batch(shell_slot(pop_e2(l))) == bi) {
                 constexpr int ex = pop_ex(l), ez = pop_ez(l);
                 constexpr int ax = ex < 0 ? -ex : ex, az = ez < 0 ? -ez : ez;
-                double s;
-                if constexpr (ex == 0 && ez == 0) s = 0.0;
-                else if constexpr (ez == 0) s = ex > 0 ? A[ax] : -A[ax];
-                else if constexpr (ex == 0) s = ez > 0 ? B[az] : -B[az];
-                else s = (ex > 0 ? A[ax] : -A[ax]) + (ez > 0 ? B[az] : -B[az]);
-                double p;
-                if constexpr (ex == 0 && ez == 0) p = g0;
-                else p = fma(fma(fma(fma(g4, s, g3), s, g2), s, g1), s, g0);
-                if constexpr (KEEP) store(L, fma(keep, load(L), p));
-                else store(L, p);
+                if constexpr (ez == 0) s[l] = ex > 0 ? A[ax] : -A[ax];
+                else if constexpr (ex == 0) s[l] = ez > 0 ? B[az] : -B[az];
+                else s[l] = (ex > 0 ? A[ax] : -A[ax]) + (ez > 0 ? B[az] : -B[az]);
+                t[l] = s[l] * s[l];
+            }
+        });
+        static_for<REST + 1, NPOP>([&](auto L) {
+            constexpr int l = decltype(L)::value;
+            constexpr int sl = shell_slot(pop_e2(l));
+            if constexpr (shell_batch(sl) == bi) {
+                ev[l] = fma(g4[sl], t[l], g2[sl]);
+                od[l] = fma(g3[sl], t[l], g1[sl]);
+            }
+        });
+        static_for<REST + 1, NPOP>([&](auto L) {
+            constexpr int l = decltype(L)::value;
+            constexpr int sl = shell_slot(pop_e2(l));
+            if constexpr (shell_batch(sl) == bi) {
+                ev[l] = fma(ev[l], t[l], g0[sl]);
+                od[l] = od[l] * s[l];
+            }
+        });
+        static_for<REST + 1, NPOP>([&](auto L) {
+            constexpr int l = decltype(L)::value;
+            if constexpr (shell_batch(shell_slot(pop_e2(l))) == bi) {
+                using LB = std::integral_constant<int, NPOP - 1 - l>;
+                if constexpr (KEEP) {
+                    store(L, fma(keep, load(L), ev[l]) + od[l]);
+                    store(LB{}, fma(keep, load(LB{}), ev[l]) - od[l]);
+                } else {
+                    store(L, ev[l] + od[l]);
+                    store(LB{}, ev[l] - od[l]);
+                }
             }
         });
     });

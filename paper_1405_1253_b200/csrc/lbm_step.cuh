@@ -124,7 +124,7 @@ __device__ __forceinline__ void scatter_site(const StepArgs &a, int i, int k, co
 // One thread per site; a block covers TX consecutive columns of TZ consecutive rows,
 // grid = (ceil(Lx/TX), ceil(Lz/TZ)).  The wall test is per row, hence warp-uniform (TX is a multiple of 32).
 template <int TX, int TZ>
-__global__ void __launch_bounds__(TX *TZ) step_kernel_site(const StepArgs a)
+__global__ void __launch_bounds__(TX *TZ, 512 / (TX * TZ)) step_kernel_site(const StepArgs a)
 {
     const int i = blockIdx.x * TX + threadIdx.x;
     const int k = blockIdx.y * TZ + threadIdx.y;

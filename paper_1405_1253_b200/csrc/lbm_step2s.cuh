@@ -40,6 +40,21 @@
 
 namespace lbm {
 
+// shared-memory access through a 32-bit shared-space address plus a compile-time byte offset (one register per base
+// instead of a 64-bit generic pointer; the offset is an immediate of the instruction)
+template <int OFF>
+__device__ __forceinline__ double lds_f64(unsigned addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(addr), "n"(OFF) : "memory");
+    return v;
+}
+template <int OFF>
+__device__ __forceinline__ void sts_f64(unsigned addr, double v)
+{
+    asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "d"(v) : "memory");
+}
+
 // split-phase barriers on mbarriers in shared memory
 __device__ __forceinline__ void mbar_init(unsigned bar, int count)
 {
@@ -141,12 +156,15 @@ __device__ __noinline__ void step2s_loader(const Step2sMaps *maps, double *stage
 // ---- producer warps: first step of intermediate rows z0-3 .. zend+2, R rows per pass ----
 template <class S>
 __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, const double *stage, unsigned bar_full,
-                                                unsigned bar_empty, unsigned bar_sfull, unsigned bar_sempty, int tid,
-                                                int x0, int z0, int ncols, int rlast, int NP)
+                                                int tid, int x0, int z0, int ncols, int rlast, int NP)
 {
+    // the four barrier arrays are consecutive (step2s_kernel): one base register
+    const unsigned bar_empty = bar_full + 8 * S::NRB, bar_sfull = bar_empty + 8 * S::NRB, bar_sempty = bar_sfull + 8 * S::NST;
     const int ar = tid / S::W1, aj = tid - ar * S::W1;
     const bool a_lane = tid < S::R * S::W1 && aj < ncols + 6;
-    const double *sp = stage + ar * S::SP + aj + 5;   // stage [l][row of the pass][span column]; span column = aj + 5 - e_lx
+    // stage [l][row of the pass][span column]; span column = aj + 5 - e_lx
+    const unsigned sp = (unsigned)__cvta_generic_to_shared(stage) + (unsigned)((ar * S::SP + aj + 5) * 8);
+    const unsigned rp0 = (unsigned)__cvta_generic_to_shared(ring) + (unsigned)(aj * 8);   // ring column of this thread
     const int c = x0 - 3 + aj;                          // this thread's column, before the periodic wrap (a1)
     const bool xwrap = c - 3 < 0 || c + 3 >= a.Lx;      // a source column wraps: the site is gathered from global memory
     int ac = c % a.Lx;
@@ -155,9 +173,9 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
     const double omega = a.omega, gtau = a.gtau, dT = a.dT;
 
     const int npass = NP + S::LEAD;
-    int b = 0;
-    unsigned use = 0;
     for (int j = 0; j < npass; ++j) {
+        const int b = j % S::NST;                       // stage buffer of this pass, and how often it was used before
+        const unsigned use = (unsigned)(j / S::NST);
         const int row = z0 - 3 + j * S::R + ar;
         const bool v = a_lane && row >= 0 && row < rlast;
         double f[NPOP];
@@ -166,10 +184,10 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
         const bool gl = v && (xwrap || row < 3 || row >= Lz - 3);
         if (gl) each_source_any(a, ac, row, [&](auto L, const double *p) { f[decltype(L)::value] = __ldcg(p); });
         mbar_wait(bar_sfull + 8 * b, use & 1u);
-        const double *sb = sp + b * S::STAGE_DOUBLES;
+        const unsigned sb = sp + (unsigned)(b * (S::STAGE_DOUBLES * 8));
         if (v && !gl) d2q37::static_for<0, NPOP>([&](auto L) {
             constexpr int l = decltype(L)::value;
-            f[l] = sb[l * S::R * S::SP - d2q37::pop_ex(l)];
+            f[l] = lds_f64<(l * S::R * S::SP - d2q37::pop_ex(l)) * 8>(sb);
         });
         // The buffer is released only after the moments have CONSUMED the 37 values (not merely after the loads were
         // issued): mbarrier.arrive does not wait for shared-memory loads in flight, and the TMA write that the
@@ -181,22 +199,20 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
             asm volatile("" : "+d"(m.m0), "+d"(m.jx), "+d"(m.jz), "+d"(m.m2));
         }
         mbar_arrive(bar_sempty + 8 * b);
-        if (++b == S::NST) { b = 0; ++use; }
         if (v) {
             const d2q37::Kinetic kin = d2q37::kinetic_from_raw(m);
             d2q37::equilibrium_blend<true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
         }
         if (j >= S::LAG) mbar_wait(bar_empty + 8 * ((j - S::LAG) % S::NRB), (unsigned)((j - S::LAG) / S::NRB) & 1u);
         if (v) {
-            double *rp = ring + aj;
             const int qrow = j * S::R + ar;             // intermediate row index within the chunk, q = row - z0 + 3
             int slot[7];                                // ring slot (in doubles) of row q, per e_z: (q mod depth) CP
 #pragma unroll                                          // (computed here, after the collision, to keep it out of its registers)
-            for (int e = 0; e < 7; ++e) slot[e] = (qrow % S::depth(e - 3)) * S::CP;
+            for (int e = 0; e < 7; ++e) slot[e] = (qrow % S::depth(e - 3)) * (S::CP * 8);   // bytes
             if (j * S::R >= 6) {
                 d2q37::static_for<0, NPOP>([&](auto L) {
                     constexpr int l = decltype(L)::value;
-                    rp[S::row_base(l) * S::CP + slot[d2q37::pop_ez(l) + 3]] = f[l];
+                    sts_f64<S::row_base(l) * S::CP * 8>(rp0 + slot[d2q37::pop_ez(l) + 3], f[l]);
                 });
             } else {
                 // warm-up: population l of intermediate row q is first read by output row q + e_lz >= 3 (q = row
@@ -204,17 +220,17 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
                 // that waits on EMPTY (no producer-producer ordering exists before pass LAG).
                 d2q37::static_for<0, NPOP>([&](auto L) {
                     constexpr int l = decltype(L)::value;
-                    if (qrow + d2q37::pop_ez(l) >= 3) rp[S::row_base(l) * S::CP + slot[d2q37::pop_ez(l) + 3]] = f[l];
+                    if (qrow + d2q37::pop_ez(l) >= 3) sts_f64<S::row_base(l) * S::CP * 8>(rp0 + slot[d2q37::pop_ez(l) + 3], f[l]);
                 });
             }
             if (z0 == 0 && row < 3) {                   // bottom wall (a3): ghost row -1-row = reversed copy of this row
                 // Only the populations that re-enter (e_z > row, read by output row e_z-1-row) are written: the
                 // other slots of rows 0..2 of a ring already belong to rows written by the next pass.
-                double *gp = rp + (2 - row) * S::CP;
+                const unsigned gp = rp0 + (unsigned)((2 - row) * (S::CP * 8));
                 d2q37::static_for<0, NPOP>([&](auto L) {
                     constexpr int l = decltype(L)::value;
                     if constexpr (d2q37::pop_ez(l) > 0)
-                        if (row < d2q37::pop_ez(l)) gp[S::row_base(l) * S::CP] = f[NPOP - 1 - l];
+                        if (row < d2q37::pop_ez(l)) sts_f64<S::row_base(l) * S::CP * 8>(gp, f[NPOP - 1 - l]);
                 });
             }
         }
@@ -225,50 +241,52 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
 // ---- consumer warps: second step of output rows z0 .. zend-1, R rows per pass ----
 template <class S>
 __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ring, unsigned bar_full,
-                                                unsigned bar_empty, int bt, int x0, int z0, int ncols, int zend, int NP)
+                                                unsigned bar_empty, int bt, int x0, int z0, int ncols, int zend)
 {
     const int br = bt / S::TX, bj = bt - br * S::TX;
     const bool b_lane = bj < ncols;
-    const double *q = ring + bj + 3;
+    const unsigned q = (unsigned)__cvta_generic_to_shared(ring) + (unsigned)((bj + 3) * 8);   // ring column of this thread
     // kernel arguments into registers once: `a` is reached through a pointer here (non-inlined role), and every
-    // global store would otherwise force its fields to be re-loaded
-    const int Lz = a.Lz;
+    // global store would otherwise force its fields to be re-loaded.  Rows are counted relative to the chunk
+    // (kq = k - z0) to keep the loop state small: the collision needs nearly all 168 registers.
+    const int zr = zend - z0;                           // output rows of the chunk
+    const int lt = a.Lz - z0;                           // kq of the first row above the top wall
     const double omega = a.omega, gtau = a.gtau, dT = a.dT;
     const long long plane = a.plane;
-    double *const out = a.dst + (long long)(z0 + br) * a.pitch + x0 + bj;    // this thread's site of pass 0, population 0
+    double *p = a.dst + (long long)(z0 + br) * a.pitch + x0 + bj;    // this thread's site of the pass, population 0
     const long long pass_stride = (long long)S::R * a.pitch;
 
-    for (int i = 0; i < NP; ++i) {
-        const int k = z0 + i * S::R + br;
-        const bool bv = b_lane && k < zend;
+    for (int i = 0; i * S::R < zr; ++i, p += pass_stride) {
+        const int kq = i * S::R + br;
+        const bool bv = b_lane && kq < zr;
         mbar_wait(bar_full + 8 * (i % S::NRB), (unsigned)(i / S::NRB) & 1u);
         double f[NPOP];
         if (bv) {
-            if (k < Lz - 3) {                           // uniform gather (bottom wall included: ghost rows)
+            if (kq < lt - 3) {                          // uniform gather (bottom wall included: ghost rows)
                 // ring slot (in doubles) of the SOURCE row k - e_z, per e_z: q = k - e_z - z0 + 3
                 int slot[7];
 #pragma unroll
-                for (int e = 0; e < 7; ++e) slot[e] = ((i * S::R + br + 3 - (e - 3)) % S::depth(e - 3)) * S::CP;
+                for (int e = 0; e < 7; ++e) slot[e] = ((kq + 3 - (e - 3)) % S::depth(e - 3)) * (S::CP * 8);   // bytes
                 d2q37::static_for<0, NPOP>([&](auto L) {
                     constexpr int l = decltype(L)::value;
-                    f[l] = q[S::row_base(l) * S::CP + slot[d2q37::pop_ez(l) + 3] - d2q37::pop_ex(l)];
+                    f[l] = lds_f64<(S::row_base(l) * S::CP - d2q37::pop_ex(l)) * 8>(q + slot[d2q37::pop_ez(l) + 3]);
                 });
             } else {                                    // top wall (a3): mirror row, opposite population
                 int off[7];
                 bool flip[7];
 #pragma unroll
                 for (int e = -3; e <= 3; ++e) {
-                    int ks = k - e;
-                    const bool fl = ks >= Lz;
-                    if (fl) ks = 2 * Lz - 1 - ks;
-                    off[e + 3] = ((ks - z0 + 3) % (fl ? S::depth(-e) : S::depth(e))) * S::CP;
+                    int ks = kq - e;                    // source row relative to the chunk
+                    const bool fl = ks >= lt;
+                    if (fl) ks = 2 * lt - 1 - ks;
+                    off[e + 3] = ((ks + 3) % (fl ? S::depth(-e) : S::depth(e))) * (S::CP * 8);
                     flip[e + 3] = fl;
                 }
                 d2q37::static_for<0, NPOP>([&](auto L) {
                     constexpr int l = decltype(L)::value;
                     constexpr int ez = d2q37::pop_ez(l);
-                    const int base = flip[ez + 3] ? S::row_base(NPOP - 1 - l) * S::CP : S::row_base(l) * S::CP;
-                    f[l] = q[base + off[ez + 3] - d2q37::pop_ex(l)];
+                    const int base = flip[ez + 3] ? S::row_base(NPOP - 1 - l) * S::CP * 8 : S::row_base(l) * S::CP * 8;
+                    f[l] = lds_f64<-d2q37::pop_ex(l) * 8>(q + base + off[ez + 3]);
                 });
             }
         }
@@ -281,8 +299,7 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
         if (bv) {
             const d2q37::Kinetic kin = d2q37::kinetic_from_raw(m);
             d2q37::equilibrium_blend<true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
-            double *p = out + i * pass_stride;          // 37 aligned stores, full 128-byte lines per warp
-            d2q37::static_for<0, NPOP>([&](auto L) {
+            d2q37::static_for<0, NPOP>([&](auto L) {     // 37 aligned stores, full 128-byte lines per warp
                 constexpr int l = decltype(L)::value;
                 st_stream(p + l * plane, f[l]);
             });
@@ -313,9 +330,9 @@ __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_cons
     __syncthreads();
     double *stage = smem2s + S::RING_DOUBLES;
     if (tid < S::NAT)
-        step2s_producer<S>(a, smem2s, stage, bar_full, bar_empty, bar_sfull, bar_sempty, tid, x0, z0, ncols, rlast, NP);
+        step2s_producer<S>(a, smem2s, stage, bar_full, tid, x0, z0, ncols, rlast, NP);
     else if (tid < S::NAT + S::NBT)
-        step2s_consumer<S>(a, smem2s, bar_full, bar_empty, tid - S::NAT, x0, z0, ncols, zend, NP);
+        step2s_consumer<S>(a, smem2s, bar_full, bar_empty, tid - S::NAT, x0, z0, ncols, zend);
     else
         step2s_loader<S>(&maps, stage, bar_sfull, bar_sempty, tid - S::NAT - S::NBT, x0, z0, NP);
 }
