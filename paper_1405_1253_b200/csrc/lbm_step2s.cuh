@@ -75,18 +75,22 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 
 template <int TX_, int R_, int NST_, int SL_>
 struct Step2sShape {
-    static constexpr int TX = TX_;                      // output columns per strip (multiple of 32)
+    static constexpr int TX = TX_;                      // output columns per strip
     static constexpr int W1 = TX_ + 6;                  // intermediate columns per strip
-    static constexpr int CP = TX_ + 8;                  // ring row pitch (doubles)
+    static constexpr int CP = (TX_ + 6 + 1) / 2 * 2;    // ring row pitch (doubles)
+    static constexpr int CW = (TX_ + 31) / 32 * 32;     // consumer threads per output row (whole warps)
     static constexpr int R = R_;                        // rows per pass
     static constexpr int NST = NST_;                    // stage buffers (passes of input in flight)
     static constexpr int SL = SL_;                      // ring slack: passes the producers may run ahead of the consumers
     static constexpr int NRB = SL_ + 1;                 // FULL / EMPTY barriers (pass i uses barrier i mod NRB)
     static constexpr int NA = (R_ * (TX_ + 6) + 31) / 32;   // producer warps (one thread per intermediate site)
-    static constexpr int NB = R_ * TX_ / 32;                // consumer warps (one thread per output site)
+    static constexpr int NB = R_ * CW / 32;                 // consumer warps (one thread per output site)
     static constexpr int NAT = NA * 32, NBT = NB * 32;
     static constexpr int NLT = 32;                          // one loader warp
-    static constexpr int SP = TX_ + 16;                     // stage row pitch = source span x0-8 .. x0+TX+7 (doubles)
+    // stage row pitch (doubles): the source span x0-6 .. x0+TX+5 padded so that a box of R rows is a multiple of 128 B
+    static constexpr int SP = (TX_ + 12 + (R_ % 2 ? 15 : 7)) / (R_ % 2 ? 16 : 8) * (R_ % 2 ? 16 : 8);
+    static constexpr int XPAD = ((SP - TX_ - 12) / 2 + 1) / 2 * 2;   // the box starts at column x0 - 6 - XPAD, kept EVEN: a box
+                                                                     // row must start on a 16-byte boundary of global memory
     static constexpr int THREADS = NAT + NBT + NLT;
     static constexpr int LEAD = 1 + 5 / R_;
     static constexpr int LAG = (7 + R_ - 1) / R_ + SL_;
@@ -102,13 +106,17 @@ struct Step2sShape {
     static constexpr size_t RING_DOUBLES = ((size_t)RING_ROWS * CP + 15) / 16 * 16;   // stage starts on a 128-byte line
     static constexpr size_t STAGE_DOUBLES = (size_t)NPOP * R_ * SP;   // per buffer
     static constexpr size_t SMEM = sizeof(double) * (RING_DOUBLES + NST_ * STAGE_DOUBLES);
-    static_assert(TX_ % 32 == 0, "a consumer warp covers 32 columns of one row");
-    static_assert(R_ >= 2 && NST_ >= 1 && NST_ <= 4, "shape");
+    static_assert(R_ >= 2 && NST_ >= 1 && NST_ <= 4 && TX_ % 2 == 0 && XPAD <= SP - TX_ - 12, "shape");
     static_assert((R_ * SP * 8) % 128 == 0 && (RING_DOUBLES * 8) % 128 == 0, "TMA box destinations are 128-byte aligned");
 };
-// Measured at 4096x8192 (profiles/r1_two_step.md): <64,2,2,0> 15.5 GLUPS; <64,3,1,0> 14.7 (no room for a second stage
-// buffer: the producers wait for the TMA round trip); <64,2,1,1> 14.2 (ring slack instead of the second buffer).
-using Step2sWide = Step2sShape<64, 2, 2, 0>;   // 5 producer + 4 consumer + 1 loader warps; ring 106 560 B + 2 x 47 360 B stage
+// Shape <TX, R, NST, SL>, measured at 4096x8192 (profiles/r1_two_step.md):
+//   <56,2,3,0> 17.3 GLUPS   4 producer + 4 consumer warps = two collisions per SM sub-partition and pass, three stage
+//                           buffers; strips of 56 columns = 14 whole 32-byte sectors per row segment
+//   <58,2,3,0> 17.2         same warp balance, but strips start off the sector grid
+//   <64,2,2,0> 16.5         5 + 4 compute warps: one sub-partition does three collisions per pass and everybody waits
+//   <60,2,3,0> 15.7         (5 producer warps again)
+//   <64,2,1,1> 14.2, <64,3,1,0> 14.7   one stage buffer: the producers wait for the TMA round trip
+using Step2sWide = Step2sShape<56, 2, 3, 0>;
 
 // Tensor maps of the source lattice (host-encoded, lbm_api.cu): rank 3 (x: Lx, z: Lz, l: 37), strides
 // (pitch, plane) doubles, box (SP, R, n) for n = 3, 5, 7 -- the populations with the same e_z are consecutive in l.
@@ -117,7 +125,7 @@ struct Step2sMaps {
 };
 
 // ---- loader warp: the gather part of the first step (a2), NST passes ahead of the producers ----
-// Seven TMA box loads per pass, one per e_z: box = span of SP source columns x0-8 .. x0+TX+3 (64-byte aligned in
+// Seven TMA box loads per pass, one per e_z: box = span of SP source columns from x0-6-XPAD (16-byte aligned in
 // global memory) x the R source rows (row - e_z) x the 3/5/7 populations with that e_z, written densely as
 // stage[l][row of the pass][span column]; the e_x shift is applied when the producers read the stage.  Coordinates
 // outside the lattice (periodic seam, walls) are zero-filled by the TMA unit and never read: the producer threads
@@ -147,7 +155,7 @@ __device__ __noinline__ void step2s_loader(const Step2sMaps *maps, double *stage
         if (lane < 7) {
             const unsigned dst = st + (unsigned)((b * S::STAGE_DOUBLES + (size_t)l0 * S::R * S::SP) * 8);
             asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                         ::"r"(dst), "l"(map), "r"(x0 - 8), "r"(z0 - 3 + j * S::R - ez), "r"(l0), "r"(bar) : "memory");
+                         ::"r"(dst), "l"(map), "r"(x0 - 6 - S::XPAD), "r"(z0 - 3 + j * S::R - ez), "r"(l0), "r"(bar) : "memory");
         }
         if (++b == S::NST) { b = 0; ++use; }
     }
@@ -162,8 +170,8 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
     const unsigned bar_empty = bar_full + 8 * S::NRB, bar_sfull = bar_empty + 8 * S::NRB, bar_sempty = bar_sfull + 8 * S::NST;
     const int ar = tid / S::W1, aj = tid - ar * S::W1;
     const bool a_lane = tid < S::R * S::W1 && aj < ncols + 6;
-    // stage [l][row of the pass][span column]; span column = aj + 5 - e_lx
-    const unsigned sp = (unsigned)__cvta_generic_to_shared(stage) + (unsigned)((ar * S::SP + aj + 5) * 8);
+    // stage [l][row of the pass][span column]; span column = aj + 3 + XPAD - e_lx
+    const unsigned sp = (unsigned)__cvta_generic_to_shared(stage) + (unsigned)((ar * S::SP + aj + 3 + S::XPAD) * 8);
     const unsigned rp0 = (unsigned)__cvta_generic_to_shared(ring) + (unsigned)(aj * 8);   // ring column of this thread
     const int c = x0 - 3 + aj;                          // this thread's column, before the periodic wrap (a1)
     const bool xwrap = c - 3 < 0 || c + 3 >= a.Lx;      // a source column wraps: the site is gathered from global memory
@@ -182,7 +190,7 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
         // sites whose sources wrap (seam strips) or reflect (wall rows, a3) bypass the stage; their loads are issued
         // before the wait so that they overlap it
         const bool gl = v && (xwrap || row < 3 || row >= Lz - 3);
-        if (gl) each_source_any(a, ac, row, [&](auto L, const double *p) { f[decltype(L)::value] = __ldcg(p); });
+        if (gl) each_source_site<true>(a, ac, row, [&](auto L, const double *p) { f[decltype(L)::value] = ld_stream(p); });
         mbar_wait(bar_sfull + 8 * b, use & 1u);
         const unsigned sb = sp + (unsigned)(b * (S::STAGE_DOUBLES * 8));
         if (v && !gl) d2q37::static_for<0, NPOP>([&](auto L) {
@@ -243,7 +251,7 @@ template <class S>
 __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ring, unsigned bar_full,
                                                 unsigned bar_empty, int bt, int x0, int z0, int ncols, int zend)
 {
-    const int br = bt / S::TX, bj = bt - br * S::TX;
+    const int br = bt / S::CW, bj = bt - br * S::CW;
     const bool b_lane = bj < ncols;
     const unsigned q = (unsigned)__cvta_generic_to_shared(ring) + (unsigned)((bj + 3) * 8);   // ring column of this thread
     // kernel arguments into registers once: `a` is reached through a pointer here (non-inlined role), and every
