@@ -30,7 +30,7 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # `ncu --set full` capture (profiles/), keyed by (workload, variant); null for anything not captured.
 # Key: (workload, steps per launch).
 NCU_TRAFFIC_BYTES = {("rt_single_4096x8192", 1): 19.814e9,    # profiles/r1_step_kernel_full.md
-                     ("rt_single_4096x8192", 2): 20.180e9}     # profiles/r1_step2_kernel_full.md
+                     ("rt_single_4096x8192", 2): 20.230e9}     # profiles/r1_step2_kernel_full.md
 
 
 def measured_peak():
@@ -244,7 +244,7 @@ def run_ours(args):
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     traffic = NCU_TRAFFIC_BYTES.get((cfg.name, int(round(spl)))) if abs(spl - round(spl)) < 1e-9 else None
     roofline = {"bound": "hbm",
-                "kernel": "step2_kernel (two fused propagate+bc+collide steps per launch)" if spl > 1.5
+                "kernel": "step2s_kernel (two fused propagate+bc+collide steps per launch)" if spl > 1.5
                 else "step_kernel_site (fused propagate+bc+collide)",
                 "achieved": achieved, "peak": peak,
                 "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",

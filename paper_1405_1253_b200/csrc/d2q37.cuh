@@ -158,12 +158,16 @@ __device__ __forceinline__ Kinetic kinetic_moments(const double (&f)[NPOP]) { re
 // thread and only one batch's coefficients are live at a time (register pressure).
 //   collision (rhs of eq. 5): keep = 1 - 1/tau, scale = rho/tau, load = post-propagate f
 //   plain equilibrium:                      keep = 0,         scale = rho
-__host__ __device__ constexpr int shell_batch(int slot)  // shells {0,1,2} {3,5,6} {4} {7}: 4-6 pairs per batch
+// WIDE = true: shells {0,1,2} {3,5,6} {4} {7}, 4-6 pairs per batch (kernels with ~168 registers); WIDE = false: one
+// shell per batch, 2-4 pairs (kernels held to 128 registers).  Batching changes the schedule only: every value is
+// the same expression either way, so the two forms are bit-identical.
+template <bool WIDE>
+__host__ __device__ constexpr int shell_batch(int slot)
 {
-    return slot <= 2 ? 0 : slot == 4 ? 2 : slot == 7 ? 3 : 1;
+    return !WIDE ? slot : slot <= 2 ? 0 : slot == 4 ? 2 : slot == 7 ? 3 : 1;
 }
 
-template <bool KEEP, class Load, class Store>
+template <bool KEEP, bool WIDE = false, class Load, class Store>
 __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&store, double keep, double scale,
                                                        double ux, double uz, double T)
 {
@@ -178,12 +182,12 @@ __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&stor
     const double B[4] = {0.0, B1, 2.0 * B1, 3.0 * B1};
     constexpr int REST = NPOP / 2;               // l = 18, e = (0, 0)
 
-    static_for<0, 4>([&](auto BI) {
+    static_for<0, (WIDE ? 4 : 8)>([&](auto BI) {
         constexpr int bi = decltype(BI)::value;
         double g0[8], g1[8], g2[8], g3[8], g4[8];                    // per shell of the batch (others never touched)
         static_for<0, 8>([&](auto S) {
             constexpr int sl = decltype(S)::value;
-            if constexpr (shell_batch(sl) == bi) {
+            if constexpr (shell_batch<WIDE>(sl) == bi) {
                 const ShellConst &c = c_shell[sl];
                 const double ws = scale * c.w;
                 g0[sl] = ws * fma(theta, fma(theta, c.k3, fma(q, c.k2, c.k1)), b0);
@@ -201,7 +205,7 @@ __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&stor
         double s[NPOP], t[NPOP], ev[NPOP], od[NPOP];
         static_for<REST + 1, NPOP>([&](auto L) {
             constexpr int l = decltype(L)::value;
-            if constexpr (shell_batch(shell_slot(pop_e2(l))) == bi) {
+            if constexpr (shell_batch<WIDE>(shell_slot(pop_e2(l))) == bi) {
                 constexpr int ex = pop_ex(l), ez = pop_ez(l);
                 constexpr int ax = ex < 0 ? -ex : ex, az = ez < 0 ? -ez : ez;
                 if constexpr (ez == 0) s[l] = ex > 0 ? A[ax] : -A[ax];
@@ -213,7 +217,7 @@ __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&stor
         static_for<REST + 1, NPOP>([&](auto L) {
             constexpr int l = decltype(L)::value;
             constexpr int sl = shell_slot(pop_e2(l));
-            if constexpr (shell_batch(sl) == bi) {
+            if constexpr (shell_batch<WIDE>(sl) == bi) {
                 ev[l] = fma(g4[sl], t[l], g2[sl]);
                 od[l] = fma(g3[sl], t[l], g1[sl]);
             }
@@ -221,14 +225,14 @@ __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&stor
         static_for<REST + 1, NPOP>([&](auto L) {
             constexpr int l = decltype(L)::value;
             constexpr int sl = shell_slot(pop_e2(l));
-            if constexpr (shell_batch(sl) == bi) {
+            if constexpr (shell_batch<WIDE>(sl) == bi) {
                 ev[l] = fma(ev[l], t[l], g0[sl]);
                 od[l] = od[l] * s[l];
             }
         });
         static_for<REST + 1, NPOP>([&](auto L) {
             constexpr int l = decltype(L)::value;
-            if constexpr (shell_batch(shell_slot(pop_e2(l))) == bi) {
+            if constexpr (shell_batch<WIDE>(shell_slot(pop_e2(l))) == bi) {
                 using LB = std::integral_constant<int, NPOP - 1 - l>;
                 if constexpr (KEEP) {
                     store(L, fma(keep, load(L), ev[l]) + od[l]);
@@ -242,11 +246,11 @@ __device__ __forceinline__ void equilibrium_blend_from(Load &&load, Store &&stor
     });
 }
 
-template <bool KEEP>
+template <bool KEEP, bool WIDE = false>
 __device__ __forceinline__ void equilibrium_blend(const double (&fin)[NPOP], double (&out)[NPOP], double keep,
                                                   double scale, double ux, double uz, double T)
 {
-    equilibrium_blend_from<KEEP>([&](auto L) { return fin[decltype(L)::value]; },
+    equilibrium_blend_from<KEEP, WIDE>([&](auto L) { return fin[decltype(L)::value]; },
                                  [&](auto L, double v) { out[decltype(L)::value] = v; }, keep, scale, ux, uz, T);
 }
 

@@ -209,7 +209,7 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
         mbar_arrive(bar_sempty + 8 * b);
         if (v) {
             const d2q37::Kinetic kin = d2q37::kinetic_from_raw(m);
-            d2q37::equilibrium_blend<true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
+            d2q37::equilibrium_blend<true, true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
         }
         if (j >= S::LAG) mbar_wait(bar_empty + 8 * ((j - S::LAG) % S::NRB), (unsigned)((j - S::LAG) / S::NRB) & 1u);
         if (v) {
@@ -306,7 +306,7 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
         mbar_arrive(bar_empty + 8 * (i % S::NRB));
         if (bv) {
             const d2q37::Kinetic kin = d2q37::kinetic_from_raw(m);
-            d2q37::equilibrium_blend<true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
+            d2q37::equilibrium_blend<true, true>(f, f, 1.0 - omega, omega * kin.rho, kin.ux, kin.uz - gtau, kin.T + dT);
             d2q37::static_for<0, NPOP>([&](auto L) {     // 37 aligned stores, full 128-byte lines per warp
                 constexpr int l = decltype(L)::value;
                 st_stream(p + l * plane, f[l]);
