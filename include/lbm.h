@@ -137,7 +137,8 @@ int lbm_steps_done(const lbm_t *h, long long *steps);
 int lbm_layout(const lbm_t *h, int *pitch, long long *plane_stride); /* in doubles */
 int lbm_kernel_launches(const lbm_t *h, long long *launches);       /* kernels launched through this handle */
 /* Step-kernel variant: 0 automatic (default), 1 one step per launch (256-thread blocks), 2 one step (128),
- * 3 two steps per launch forced (lbm_step2.cuh).  All give bit-identical results. */
+ * 3 two steps per launch forced (lbm_step2s.cuh; automatic picks it from about 512x1024 up).  All give
+ * bit-identical results. */
 int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel, or 0 = automatic */
 /* D2Q37 tables as the library uses them (host outputs, any may be NULL): e_x[37], e_z[37], w[37], r. */
