@@ -106,7 +106,7 @@ struct Step2sShape {
     static constexpr size_t RING_DOUBLES = ((size_t)RING_ROWS * CP + 15) / 16 * 16;   // stage starts on a 128-byte line
     static constexpr size_t STAGE_DOUBLES = (size_t)NPOP * R_ * SP;   // per buffer
     static constexpr size_t SMEM = sizeof(double) * (RING_DOUBLES + NST_ * STAGE_DOUBLES);
-    static_assert(R_ >= 2 && NST_ >= 1 && NST_ <= 4 && TX_ % 2 == 0 && XPAD <= SP - TX_ - 12, "shape");
+    static_assert(R_ >= 1 && NST_ >= 1 && NST_ <= 4 && TX_ % 2 == 0 && XPAD <= SP - TX_ - 12, "shape");
     static_assert((R_ * SP * 8) % 128 == 0 && (RING_DOUBLES * 8) % 128 == 0, "TMA box destinations are 128-byte aligned");
 };
 // Shape <TX, R, NST, SL>, measured at 4096x8192 (profiles/r1_two_step.md):
@@ -116,7 +116,14 @@ struct Step2sShape {
 //   <64,2,2,0> 16.5         5 + 4 compute warps: one sub-partition does three collisions per pass and everybody waits
 //   <60,2,3,0> 15.7         (5 producer warps again)
 //   <64,2,1,1> 14.2, <64,3,1,0> 14.7   one stage buffer: the producers wait for the TMA round trip
-using Step2sWide = Step2sShape<56, 2, 3, 0>;
+//   <112,1,2,0> 16.8, <120,1,1,0> 14.8  one row per pass, wide strips (5 % halo work instead of 11 %), fewer buffers
+#ifndef S2S_TX   // shape experiments: -DS2S_TX=.. -DS2S_R=.. -DS2S_NST=.. -DS2S_SL=..
+#define S2S_TX 56
+#define S2S_R 2
+#define S2S_NST 3
+#define S2S_SL 0
+#endif
+using Step2sWide = Step2sShape<S2S_TX, S2S_R, S2S_NST, S2S_SL>;
 
 // Tensor maps of the source lattice (host-encoded, lbm_api.cu): rank 3 (x: Lx, z: Lz, l: 37), strides
 // (pitch, plane) doubles, box (SP, R, n) for n = 3, 5, 7 -- the populations with the same e_z are consecutive in l.
@@ -204,6 +211,9 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
         d2q37::RawMoments m;
         if (v) {
             m = d2q37::raw_moments(f);
+            // keeps the arrive below the sums in the instruction stream: a DADD cannot issue before its operands
+            // have returned from shared memory, and a warp issues in order (tests/test_library_cpu.py checks the
+            // order in the SASS; making the barrier address depend on the sums instead costs 3.5 %)
             asm volatile("" : "+d"(m.m0), "+d"(m.jx), "+d"(m.jz), "+d"(m.m2));
         }
         mbar_arrive(bar_sempty + 8 * b);

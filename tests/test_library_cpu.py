@@ -109,3 +109,48 @@ def test_growth_rate_host_function_matches_oracle_and_closed_form(lib, orc):
         pkg.growth_rate(tq[::-1].copy(), tq, 1e-4, 0.05)      # times must increase
     with pytest.raises(pkg.LbmError):
         pkg.growth_rate(tq, tq, 0.0, 0.05)
+
+
+def test_two_step_kernel_releases_buffers_only_after_consuming_them():
+    """Guards the fix of the hand-off race of lbm_step2s.cuh (profiles/r1_two_step.md, section 4) against compiler
+    scheduling: in the SASS of step2s_kernel every gather of 37 populations from shared memory (a run of LDS) must be
+    followed by the moment sums (>= 60 DADD, which cannot issue before the loaded values have returned) BEFORE the
+    next mbarrier arrive (SYNCS.ARRIVE) that releases the buffer.  Skipped where cuobjdump is not installed."""
+    import shutil
+    import subprocess
+    from paper_1405_1253_b200 import binding
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", binding.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    ops, inside = [], False
+    for line in sass.splitlines():
+        if "Function :" in line:
+            inside = "step2s_kernel" in line
+        elif inside and "/*" in line and "*/" in line:
+            body = line.split("*/", 1)[1].strip()
+            tok = body.split()
+            if not tok:
+                continue
+            op = tok[1] if tok[0].startswith("@") and len(tok) > 1 else tok[0]
+            ops.append(op.rstrip(";"))
+    assert ops, "step2s_kernel not found in the library"
+    gathers = 0
+    i = 0
+    while i < len(ops):
+        if ops[i].startswith("LDS"):
+            j, n_lds = i, 0
+            while j < len(ops) and not ops[j].startswith(("DADD", "SYNCS")):   # the run of loads (with address arithmetic)
+                n_lds += ops[j].startswith("LDS")
+                j += 1
+            if n_lds >= 30:
+                gathers += 1
+                k, n_dadd = j, 0
+                while k < len(ops) and not ops[k].startswith("SYNCS.ARRIVE"):
+                    n_dadd += ops[k].startswith("DADD")
+                    k += 1
+                assert k < len(ops), "no release after a gather"
+                assert n_dadd >= 60, f"buffer released after only {n_dadd} DADD following a gather of {n_lds} LDS"
+            i = j
+        i += 1
+    assert gathers >= 2, f"expected the producers' and the consumers' gathers, found {gathers}"
