@@ -25,6 +25,7 @@ sys.path.insert(0, ROOT)
 import synthetic_inputs as si  # noqa: E402
 
 BYTES_PER_SITE = 592          # 37 x 8 B read + 37 x 8 B written per site per step
+FLOPS_PER_SITE = 559          # FP64 flops of one collision, FMA = 2: 196 DFMA + 89 DADD + 78 DMUL in the SASS
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel at 4096x8192, from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, variant); null for anything not captured.
@@ -216,6 +217,7 @@ def run_ours(args):
     host_in = [x.cpu().pin_memory() for x in (rho, ux, uz - 0.5 * g, T - 0.125 * g * g)]  # kinetic fields
     host_out = tuple(torch.empty_like(x).pin_memory() for x in host_in)
     del rho, ux, uz, T
+    fp64_peak = max(pkg.fp64_peak() for _ in range(2))                  # TFLOP/s, DFMA chains on all SMs (clock under load)
     e2e_steps = args.e2e_steps or args.steps
     lat.run_host(*host_in, n=min(3, e2e_steps), outs=host_out)          # warm-up (allocates staging)
     barrier()
@@ -251,7 +253,12 @@ def run_ours(args):
                 "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "bytes_per_site_step": BYTES_PER_SITE, "steps_per_launch": spl, "launches": step_launches,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": launch_ms, "traffic": traffic,
-                "dram_gbs": (traffic / (launch_ms * 1e-3) / 1e9) if traffic else None}
+                "dram_gbs": (traffic / (launch_ms * 1e-3) / 1e9) if traffic else None,
+                # the other candidate roof (north_star): FP64.  Algorithmic flops of the collision x site-steps / s
+                # against the vector-FP64 rate a DFMA-chain probe reaches on this GPU in this process.
+                "fp64": {"flops_per_site_step": FLOPS_PER_SITE, "achieved_tflops": FLOPS_PER_SITE * sites * spl / (launch_ms * 1e-3) / 1e12,
+                         "peak_tflops": fp64_peak, "peak_kind": "measured: lbm_fp64_peak (8 DFMA chains/thread, all SMs)",
+                         "frac": FLOPS_PER_SITE * sites * spl / (launch_ms * 1e-3) / 1e12 / fp64_peak}}
     cpu = None
     if not args.no_cpu_baseline:
         v, cores, sample = oracle_sample_rate(cfg, args.cpu_budget)

@@ -136,6 +136,11 @@ int lbm_run_host(lbm_t *h, const double *rho_in, const double *ux_in, const doub
 int lbm_steps_done(const lbm_t *h, long long *steps);
 int lbm_layout(const lbm_t *h, int *pitch, long long *plane_stride); /* in doubles */
 int lbm_kernel_launches(const lbm_t *h, long long *launches);       /* kernels launched through this handle */
+/* Measurement aid ("no FP64 entry in MEASURED_PEAKS.json -- measure with a DFMA-chain microbenchmark"):
+ * runs 8 independent DFMA chains per thread on every SM for `iters` rounds (0 = default), times them with CUDA
+ * events on `stream` and returns the vector-FP64 rate in TFLOP/s (FMA = 2 flops) in HOST *tflops.  Not part of the
+ * time step.  Synchronises `stream`. */
+int lbm_fp64_peak(double *tflops, int iters, void *stream);
 /* Step-kernel variant: 0 automatic (default), 1 one step per launch (256-thread blocks), 2 one step (128),
  * 3 two steps per launch forced (lbm_step2s.cuh; automatic picks it from about 512x1024 up).  All give
  * bit-identical results. */

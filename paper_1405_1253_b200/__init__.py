@@ -35,6 +35,13 @@ def growth_rate(t, L, g: float, At: float):
     return out
 
 
+def fp64_peak(iters: int = 0, stream=None) -> float:
+    """Vector-FP64 rate of this GPU in TFLOP/s from a DFMA-chain probe (lbm_fp64_peak; measurement aid)."""
+    out = C.c_double(0.0)
+    binding.check(binding.load().lbm_fp64_peak(C.byref(out), int(iters), _stream_ptr(stream)))
+    return out.value
+
+
 def _stream_ptr(stream):
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()

@@ -18,7 +18,7 @@ SYMBOLS = [
     "lbm_buffer_bytes", "lbm_create", "lbm_destroy", "lbm_init_rt", "lbm_init_equilibrium",
     "lbm_set_populations", "lbm_get_populations", "lbm_set_populations_host", "lbm_get_populations_host",
     "lbm_step", "lbm_moments", "lbm_mixing_widths", "lbm_profiles", "lbm_growth_rate", "lbm_totals", "lbm_run_host", "lbm_steps_done",
-    "lbm_layout", "lbm_kernel_launches", "lbm_set_variant", "lbm_set_zchunk", "lbm_tables", "lbm_last_error",
+    "lbm_layout", "lbm_kernel_launches", "lbm_fp64_peak", "lbm_set_variant", "lbm_set_zchunk", "lbm_tables", "lbm_last_error",
 ]
 
 
@@ -69,6 +69,7 @@ def load():
     L.lbm_steps_done.argtypes = [vp, C.POINTER(C.c_longlong)]
     L.lbm_layout.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
     L.lbm_kernel_launches.argtypes = [vp, C.POINTER(C.c_longlong)]
+    L.lbm_fp64_peak.argtypes = [dp, C.c_int, vp]
     L.lbm_set_variant.argtypes = [vp, C.c_int]
     L.lbm_set_zchunk.argtypes = [vp, C.c_int]
     L.lbm_tables.argtypes = [C.POINTER(C.c_int), C.POINTER(C.c_int), dp, dp]

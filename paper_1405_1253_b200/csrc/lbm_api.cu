@@ -401,6 +401,36 @@ int lbm_growth_rate(int n, const double *t, const double *L, double g, double At
     return LBM_OK;
 }
 
+int lbm_fp64_peak(double *tflops, int iters, void *stream)
+{
+    if (!tflops) return fail(LBM_ERR_INVALID, "lbm_fp64_peak: null output");
+    if (iters <= 0) iters = 4096;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(LBM_ERR_NODEVICE, "lbm_fp64_peak: no CUDA device");
+    }
+    double *sink = nullptr;
+    CUDA_TRY(cudaMalloc(&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    const int blocks = prop.multiProcessorCount * 4;    // 4 x 256 threads = 8 warps per sub-partition
+    lbm::fp64_peak_kernel<<<blocks, 256, 0, st>>>(sink, 16, 1.0000001, 1e-9);   // warm-up
+    CUDA_TRY(cudaEventRecord(e0, st));
+    lbm::fp64_peak_kernel<<<blocks, 256, 0, st>>>(sink, iters, 1.0000001, 1e-9);
+    CUDA_TRY(cudaEventRecord(e1, st));
+    CUDA_TRY(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    CUDA_TRY(cudaGetLastError());
+    *tflops = 2.0 * 16.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+    return LBM_OK;
+}
+
 int lbm_totals(lbm_t *h, double *out4, void *stream)
 {
     NEED(h);

@@ -244,4 +244,22 @@ __global__ void __launch_bounds__(RED_T) final_totals_kernel(const double *__res
     }
 }
 
+// FP64 peak probe (include/lbm.h lbm_fp64_peak): 8 independent DFMA chains per thread, 8 warps per SM sub-partition.
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters, double a, double b)
+{
+    double x[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x[j] = a * (threadIdx.x + j);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) x[j] = fma(x[j], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) s += x[j];
+    if (s == 12345.678) sink[0] = s;      // never true: keeps the chains alive
+}
+
 }  // namespace lbm

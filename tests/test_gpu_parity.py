@@ -222,3 +222,10 @@ def test_two_step_kernel_is_bitwise_equal_to_single_steps(pkg, orc, Lx, Lz, zchu
     assert b.steps_done == n and torch.equal(fa, fb)
     assert _rel(fb.cpu().numpy(), orc.step(f0, 0.66, 3e-4, nsteps=n)) < POP_RTOL
     a.close(); b.close()
+
+
+def test_fp64_peak_probe_is_plausible(pkg):
+    """lbm_fp64_peak (DFMA chains on all SMs) backs the FP64 side of the roofline in bench.py: B200 is specified
+    at 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s; anything far off means a broken probe or a throttled GPU."""
+    v = max(pkg.fp64_peak() for _ in range(3))
+    assert 15.0 < v < 45.0, v

@@ -22,7 +22,7 @@ def lib():
 def test_library_exports_every_declared_symbol(lib):
     from paper_1405_1253_b200 import binding
     header = open(os.path.join(ROOT, "include", "lbm.h")).read()
-    declared = set(re.findall(r"\b(lbm_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(lbm_[a-z0-9_]+)\s*\(", header))
     assert declared == set(binding.SYMBOLS)
     for name in declared:
         assert hasattr(lib, name), name
