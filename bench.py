@@ -30,7 +30,7 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel at 4096x8192, from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, variant); null for anything not captured.
 # Key: (workload, steps per launch).
-NCU_TRAFFIC_BYTES = {("rt_single_4096x8192", 1): 19.814e9,    # profiles/r1_step_kernel_full.md
+NCU_TRAFFIC_BYTES = {("rt_single_4096x8192", 1): 19.836e9,    # profiles/r1_step_kernel_full.md
                      ("rt_single_4096x8192", 2): 20.230e9}     # profiles/r1_step2_kernel_full.md
 
 
