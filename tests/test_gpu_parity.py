@@ -67,16 +67,20 @@ def test_config1_100_steps_population_parity(pkg, orc, variant):
     lat.close()
 
 
+@pytest.mark.parametrize("variant", [0, 3])
 @pytest.mark.parametrize("Lx,Lz,steps", [(7, 6, 5), (33, 9, 12), (130, 70, 20), (257, 40, 10), (520, 18, 7)])
-def test_ragged_and_tiny_lattices_from_identical_populations(pkg, orc, Lx, Lz, steps):
+def test_ragged_and_tiny_lattices_from_identical_populations(pkg, orc, Lx, Lz, steps, variant):
     """Same starting populations on both sides (uploaded), odd sizes: minimum lattice, ragged block tails,
-    lattices where every row is a wall row, several blocks per row."""
+    lattices where every row is a wall row, several blocks per row -- with the automatic kernel choice (one step
+    per launch at these sizes) and with the two-step kernel forced (strips narrower than 56 columns, odd widths,
+    an odd last step)."""
     rng = np.random.default_rng(Lx * 1000 + Lz)
     rho = 1 + 0.05 * rng.uniform(-1, 1, (Lz, Lx)); T = 1 + 0.05 * rng.uniform(-1, 1, (Lz, Lx))
     ux = 0.03 * rng.uniform(-1, 1, (Lz, Lx)); uz = 0.03 * rng.uniform(-1, 1, (Lz, Lx))
     f0 = orc.init_equilibrium(rho, ux, uz, T) * (1 + 0.01 * rng.uniform(-1, 1, (37, Lz, Lx)))
     import torch
     lat = pkg.Lattice(Lx, Lz, 0.63, 2e-4)
+    lat.set_variant(variant)
     lat.set_populations(torch.from_numpy(f0))                 # host path
     assert np.array_equal(lat.get_populations(host=True).numpy(), f0)   # layout round trip is bit exact
     lat.step(steps)
@@ -229,3 +233,25 @@ def test_fp64_peak_probe_is_plausible(pkg):
     at 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s; anything far off means a broken probe or a throttled GPU."""
     v = max(pkg.fp64_peak() for _ in range(3))
     assert 15.0 < v < 45.0, v
+
+
+@pytest.mark.parametrize("tau,g", [(0.51, 0.0), (2.0, 1e-3), (0.8, 0.0)])
+def test_two_step_kernel_parameter_extremes_against_oracle(pkg, orc, tau, g):
+    """Relaxation close to the stability limit, over-relaxation, no gravity: 30 steps of the two-step kernel on a
+    lattice with a ragged strip (300 = 5 x 56 + 20) and chunk tail, every population against the oracle."""
+    import torch
+    Lx, Lz = 300, 100
+    rng = np.random.default_rng(77)
+    rho = 1 + 0.02 * rng.uniform(-1, 1, (Lz, Lx)); T = 1 + 0.02 * rng.uniform(-1, 1, (Lz, Lx))
+    ux = 0.01 * rng.uniform(-1, 1, (Lz, Lx)); uz = 0.01 * rng.uniform(-1, 1, (Lz, Lx))
+    f0 = orc.init_equilibrium(rho, ux, uz, T)
+    lat = pkg.Lattice(Lx, Lz, tau, g)
+    lat.set_variant(3); lat.set_zchunk(28)
+    lat.set_populations(torch.from_numpy(f0).cuda())
+    lat.step(30)
+    got = lat.get_populations(host=True).numpy()
+    ref = orc.step(f0, tau, g, nsteps=30)
+    assert _rel(got, ref) < POP_RTOL
+    tg, tr = lat.totals(), orc.totals(ref)
+    assert abs(tg[0] / tr[0] - 1) < TOT_RTOL and abs(tg[3] / tr[3] - 1) < TOT_RTOL
+    lat.close()
