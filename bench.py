@@ -31,7 +31,7 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # `ncu --set full` capture (profiles/), keyed by (workload, variant); null for anything not captured.
 # Key: (workload, steps per launch).
 NCU_TRAFFIC_BYTES = {("rt_single_4096x8192", 1): 19.836e9,    # profiles/r1_step_kernel_full.md
-                     ("rt_single_4096x8192", 2): 20.230e9}     # profiles/r1_step2_kernel_full.md
+                     ("rt_single_4096x8192", 2): 20.230e9}     # profiles/r1_step2s_kernel_full.md
 
 
 def measured_peak():
@@ -237,7 +237,7 @@ def run_ours(args):
 
     peak, peak_kind = measured_peak()
     # Dominant kernel: the step kernel.  Algorithmic bytes per launch = 592 B/site/step x sites x
-    # the steps one launch advances (1: step_kernel_site, 2: step2_kernel, which keeps the intermediate lattice
+    # the steps one launch advances (1: step_kernel_site, 2: step2s_kernel, which keeps the intermediate lattice
     # in shared memory, so its DRAM traffic -- `traffic`, from ncu -- is about half its algorithmic bytes and
     # `frac` can exceed 1: DESIGN.md section 6).  Launch duration = CUDA-event time of the K steps / launches.
     spl = args.steps / max(step_launches, 1)
