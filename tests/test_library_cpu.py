@@ -111,7 +111,7 @@ def test_growth_rate_host_function_matches_oracle_and_closed_form(lib, orc):
         pkg.growth_rate(tq, tq, 0.0, 0.05)
 
 
-def test_two_step_kernel_releases_buffers_only_after_consuming_them():
+def test_two_step_kernel_releases_buffers_only_after_consuming_them(lib):
     """Guards the fix of the hand-off race of lbm_step2s.cuh (profiles/r1_two_step.md, section 4) against compiler
     scheduling: in the SASS of step2s_kernel every gather of 37 populations from shared memory (a run of LDS) must be
     followed by the moment sums (>= 60 DADD, which cannot issue before the loaded values have returned) BEFORE the
