@@ -96,9 +96,12 @@ def oracle_sample_rate(cfg, budget_s: float, threads: int | None = None):
     rows = 64
     sub = si.scaled(cfg, cfg.Lx, rows)
     f = orc.init_rt(sub.Lx, sub.Lz, sub.g, si.DEFAULT_SEED, **sub.rt_args())
-    t0 = time.perf_counter(); f = orc.step(f, sub.tau, sub.g, nsteps=1); t1 = time.perf_counter() - t0
-    n = max(2, int(budget_s / max(t1, 1e-6)))
-    t0 = time.perf_counter(); orc.step(f, sub.tau, sub.g, nsteps=n); dt = time.perf_counter() - t0
+    f = orc.step(f, sub.tau, sub.g, nsteps=2)                     # untimed: thread start-up, page faults
+    n, dt, batch = 0, 0.0, 8
+    while dt < budget_s:                                          # doubling batches until the budget is spent
+        t0 = time.perf_counter(); f = orc.step(f, sub.tau, sub.g, nsteps=batch); dt += time.perf_counter() - t0
+        n += batch
+        batch = min(2 * batch, max(8, int(n / max(dt, 1e-6) * max(budget_s - dt, 0.0)) + 1))
     mlups = sub.Lx * rows * n / dt / 1e6
     return mlups, cores, f"{sub.Lx}x{rows} slab of {cfg.name} around the interface, {n} steps, {dt:.1f} s"
 
