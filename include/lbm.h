@@ -145,7 +145,7 @@ int lbm_fp64_peak(double *tflops, int iters, void *stream);
  * 3 two steps per launch forced (lbm_step2s.cuh; automatic picks it from about 512x1024 up).  All give
  * bit-identical results. */
 int lbm_set_variant(lbm_t *h, int variant);
-int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel, or 0 = automatic */
+int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel (>= 3), or 0 = automatic */
 /* D2Q37 tables as the library uses them (host outputs, any may be NULL): e_x[37], e_z[37], w[37], r. */
 int lbm_tables(int *ex, int *ez, double *w, double *r);
 const char *lbm_last_error(void);

@@ -496,7 +496,9 @@ int lbm_kernel_launches(const lbm_t *h, long long *launches)
 int lbm_set_zchunk(lbm_t *h, int rows)
 {
     NEED(h);
-    if (rows < 0) return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be 0 (automatic) or positive (got %d)", rows);
+    // chunks above the first must start at row >= 3: only the chunk at z0 = 0 builds the bottom wall's ghost rows
+    if (rows < 0 || rows == 1 || rows == 2)
+        return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be 0 (automatic) or >= 3 (got %d)", rows);
     h->zchunk = rows;
     return LBM_OK;
 }

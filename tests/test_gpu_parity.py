@@ -204,7 +204,8 @@ def test_step_is_cuda_graph_capturable(pkg):
 
 @pytest.mark.parametrize("Lx,Lz,zchunk,n", [(7, 6, 3, 4), (33, 9, 3, 5), (64, 128, 192, 6), (130, 70, 9, 7),
                                             (257, 40, 15, 4), (520, 18, 126, 2), (70, 64, 12, 10), (191, 37, 21, 3),
-                                            (130, 70, 7, 4), (200, 50, 10, 6), (128, 31, 5, 2)])
+                                            (130, 70, 7, 4), (200, 50, 10, 6), (128, 31, 5, 2), (64, 20, 3, 2), (100, 12, 4, 4),
+                                            (57, 6, 4, 2), (113, 7, 3, 6)])
 @pytest.mark.parametrize("fused_variant", [3])
 def test_two_step_kernel_is_bitwise_equal_to_single_steps(pkg, orc, Lx, Lz, zchunk, n, fused_variant):
     """Variant 3 fuses two time steps per launch through shared memory (lbm_step2s.cuh: TMA loader, producer and
@@ -224,6 +225,9 @@ def test_two_step_kernel_is_bitwise_equal_to_single_steps(pkg, orc, Lx, Lz, zchu
         lat.step(n)
     fa, fb = a.get_populations(), b.get_populations()
     assert b.steps_done == n and torch.equal(fa, fb)
+    for bad in (1, 2, -3):                      # chunks must be at least as tall as the wall zone
+        with pytest.raises(pkg.LbmError):
+            b.set_zchunk(bad)
     assert _rel(fb.cpu().numpy(), orc.step(f0, 0.66, 3e-4, nsteps=n)) < POP_RTOL
     a.close(); b.close()
 
