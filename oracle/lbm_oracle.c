@@ -30,6 +30,15 @@
  *                                  geometry constants and the perturbation RNG are READINGS:
  *                                  parity with the authors' exact initial field is UNPINNED.
  *   orc_mixing_widths      pinned: closed form on step/tanh profiles (eq. 8, 9, 12).
+ *   orc_bc_isothermal      pinned (tests/test_oracle_walls.py): after a step the three wall rows carry u^(H) = 0
+ *                                  and T^(H) = T_wall to rounding; mass conserved to rounding; rest state at
+ *                                  T_wall is a fixed point; slowest shear mode decays as between no-slip
+ *                                  planes at the innermost imposed rows; steady conduction between walls at
+ *                                  different temperatures is a linear T(z) (uniform conductivity at uniform
+ *                                  pressure) carrying the flux k dT/dz with k = c_p (tau - 1/2) p / r^2.
+ *                                  The rule itself is a READING of "rigid boundary conditions ... adjusts
+ *                                  population values at sites with z = 0, 1, 2": parity with
+ *                                  the authors' wall scheme is UNPINNED (reading 19).
  *
  * Conventions: sites (i,k), i = 0..Lx-1 (x, periodic), k = 0..Lz-1
  * (z, up); arrays are dense f[l][k][i], x fastest; population order: ascending e_z, then
@@ -293,6 +302,57 @@ void orc_collide(const double *fs, double *fnew, int Lx, int Lz, double tau, dou
             for (int l = 0; l < NPOP; ++l)
                 fnew[l * plane + s] = fl[l] - (1.0 / tau) * (fl[l] - feq[l]);
         }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Isothermal no-slip walls, wall_kind = 1 (reading 19).  PAPER.md:114: "Step bc
+ * executes after propagate in order to enforce boundary conditions at the top and bottom of
+ * the cell; it adjusts population values at sites with coordinates z = 0, 1, 2 and
+ * z = Lz-3, Lz-2 and Lz-1"; the paper gives no formula, its references impose the wall
+ * temperature and zero velocity on the three rows.  Reading: after propagate (whose wall-
+ * crossing gathers are filled by the bounce-back rule of orc_propagate, which conserves
+ * mass), every site of the three rows next to a wall has the EQUILIBRIUM PART of its
+ * populations moved to the wall state, keeping density and non-equilibrium part:
+ *   (rho*, u*, T*) = moments (eq. 7) of the post-propagate populations fs at the site;
+ *   fs_l  <-  fs_l - f_eq_l(rho*, u*, T*) + f_eq_l(rho*, u_w, T_w)
+ *   u_w = -g_vec dt/2 = (0, +g/2),   T_w = T_wall - dt^2 g^2 / (4 D),
+ * i.e. the kinetic moments that PAPER.md:94 maps to the hydrodynamic fields u^(H) = 0,
+ * T^(H) = T_wall.  By the closure of eq. 7 the adjusted populations have exactly the moments
+ * (rho*, u_w, T_w); collide then runs unchanged on them.  T_bot applies to rows 0..2, T_top
+ * to rows Lz-3..Lz-1.
+ * ------------------------------------------------------------------------------------- */
+void orc_bc_isothermal(double *fs, int Lx, int Lz, double g, double T_bot, double T_top)
+{
+    ensure_tables();
+    const size_t plane = (size_t)Lx * (size_t)Lz;
+    for (int side = 0; side < 2; ++side)
+        for (int j = 0; j < 3; ++j) {
+            const int k = side == 0 ? j : Lz - 1 - j;
+            const double T_wall = side == 0 ? T_bot : T_top;
+            const double uw_x = 0.0, uw_z = 0.5 * g;
+            const double Tw = T_wall - g * g / (4.0 * DIM);
+            for (int i = 0; i < Lx; ++i) {
+                const size_t s = (size_t)k * Lx + i;
+                double fl[NPOP], feq_own[NPOP], feq_wall[NPOP], rho, ux, uz, T;
+                for (int l = 0; l < NPOP; ++l) fl[l] = fs[l * plane + s];
+                site_moments(fl, &rho, &ux, &uz, &T);
+                orc_feq(rho, ux, uz, T, feq_own);
+                orc_feq(rho, uw_x, uw_z, Tw, feq_wall);
+                for (int l = 0; l < NPOP; ++l) fs[l * plane + s] = fl[l] - feq_own[l] + feq_wall[l];
+            }
+        }
+}
+
+/* n time steps with a choice of wall rule: wall_kind 0 = bounce-back only (reading 9),
+ * 1 = bounce-back fill followed by the isothermal adjustment above (reading 19). */
+void orc_step_walls(double *f, double *tmp, int Lx, int Lz, double tau, double g, int nsteps, int wall_kind,
+                    double T_bot, double T_top)
+{
+    for (int n = 0; n < nsteps; ++n) {
+        orc_propagate(f, tmp, Lx, Lz, 0, +1);
+        if (wall_kind == 1) orc_bc_isothermal(tmp, Lx, Lz, g, T_bot, T_top);
+        orc_collide(tmp, f, Lx, Lz, tau, g);
+    }
 }
 
 /* n time steps: propagate -> bc -> collide; f is updated in place, tmp is

@@ -48,6 +48,9 @@ def lib():
         L.orc_propagate.argtypes = [_dp, _dp, C.c_int, C.c_int, C.c_int, C.c_int]
         L.orc_collide.argtypes = [_dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double]
         L.orc_step.argtypes = [_dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int]
+        L.orc_bc_isothermal.argtypes = [_dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]
+        L.orc_step_walls.argtypes = [_dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double,
+                                     C.c_double]
         L.orc_moments.argtypes = [_dp, C.c_int, C.c_int, C.c_double] + [C.c_void_p] * 4
         L.orc_totals.argtypes = [_dp, C.c_int, C.c_int, _dp]
         L.orc_mixing_widths.argtypes = (
@@ -111,13 +114,27 @@ def collide(fs: np.ndarray, tau: float, g: float) -> np.ndarray:
     return out
 
 
-def step(f: np.ndarray, tau: float, g: float, nsteps: int = 1, periodic_z: bool = False) -> np.ndarray:
-    """Returns the state after nsteps x (propagate, bc, collide); the input is not modified."""
+def step(f: np.ndarray, tau: float, g: float, nsteps: int = 1, periodic_z: bool = False, wall_kind: int = 0,
+         T_bot: float = 1.0, T_top: float = 1.0) -> np.ndarray:
+    """Returns the state after nsteps x (propagate, bc, collide); the input is not modified.
+    wall_kind 1 = isothermal no-slip walls at T_bot / T_top (orc_step_walls)."""
     _, Lz, Lx = f.shape
     cur = np.array(f, dtype=np.float64, order="C", copy=True)
     tmp = np.empty_like(cur)
-    lib().orc_step(cur, tmp, Lx, Lz, tau, g, int(nsteps), int(periodic_z))
+    if wall_kind == 0:
+        lib().orc_step(cur, tmp, Lx, Lz, tau, g, int(nsteps), int(periodic_z))
+    else:
+        assert not periodic_z
+        lib().orc_step_walls(cur, tmp, Lx, Lz, tau, g, int(nsteps), int(wall_kind), T_bot, T_top)
     return cur
+
+
+def bc_isothermal(fs: np.ndarray, g: float, T_bot: float, T_top: float) -> np.ndarray:
+    """The wall adjustment of reading 19 applied to post-propagate populations (returns a copy)."""
+    _, Lz, Lx = fs.shape
+    out = np.array(fs, dtype=np.float64, order="C", copy=True)
+    lib().orc_bc_isothermal(out, Lx, Lz, g, T_bot, T_top)
+    return out
 
 
 def moments(f: np.ndarray, g: float):
