@@ -12,7 +12,8 @@
  * [37][Lz][Lx].  Population order: ascending e_z, then ascending e_x over all integer e with |e|^2 <= 10
  * (l = 0 is (-1,-3), l = 18 is (0,0), l = 36 is (1,3)); the opposite of l is 36 - l.  dt = 1, c_l = r e_l,
  * gravity (0,-g), g >= 0.  "device" pointers are CUDA device memory of the current device, "host" pointers
- * ordinary host memory.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ * ordinary host memory.  A handle belongs to the device that was current in lbm_create; every call that touches
+ * the device returns LBM_ERR_INVALID if another device is current.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
  *
  * Errors.  Every call returns 0 on success or a negative lbm_status; no exception crosses the boundary;
  * lbm_last_error() returns a thread-local message for the last failing call.
@@ -41,16 +42,25 @@ typedef enum {
 typedef struct lbm_handle lbm_t;
 
 /* Model parameters and storage.  tau = tau_LB/dt of eq. 5 (> 1/2); g = |gravity| of eq. 3/6 (>= 0).
- * wall_kind: 0 = half-way bounce-back through velocity-reversed mirror rows (reading 9).
+ * wall_kind ("rigid boundary conditions" on rows 0..2 and Lz-3..Lz-1; the paper gives no formula):
+ *   0 = half-way bounce-back through velocity-reversed mirror rows (reading 9): adiabatic, no-slip;
+ *   1 = isothermal no-slip walls (reading 19): after propagate (wall-crossing gathers filled as for 0) the
+ *       equilibrium part of the populations of the three rows next to each wall is moved to the wall state
+ *       u^(H) = 0, T^(H) = T_wall_bottom / T_wall_top, density and non-equilibrium part kept; then collide.
  * pop_buf0/pop_buf1: device buffers of at least lbm_buffer_bytes(Lx,Lz) bytes each, 256-byte aligned;
- * they hold the two lattice copies (prv/nxt of PAPER.md:110) in the library's padded SoA layout. */
+ * they hold the two lattice copies (prv/nxt of PAPER.md:110) in the library's padded SoA layout.
+ * pop_buf1 = NULL selects IN-PLACE streaming with ONE lattice copy (two copies "require more
+ * memory"): two alternating one-step kernels that write every result back into the slots they read; results are
+ * bit-identical to the two-copy path; the two-step kernel (variant 3) is not available. */
 typedef struct {
     double tau;
     double g;
     int wall_kind;
     void *pop_buf0; /* device */
-    void *pop_buf1; /* device */
+    void *pop_buf1; /* device, or NULL: one copy, in-place streaming */
     size_t buf_bytes;
+    double T_wall_bottom; /* wall_kind 1 only */
+    double T_wall_top;    /* wall_kind 1 only */
 } lbm_params;
 
 /* Rayleigh-Taylor initial state, eq. 1-2 with tanh-smoothed jumps.
@@ -72,9 +82,36 @@ typedef struct {
 /* Bytes each population buffer must have for an Lx x Lz lattice (padded rows, 37 planes); 0 if invalid. */
 size_t lbm_buffer_bytes(int Lx, int Lz);
 
-/* Creates a handle. Errors: Lx < 7, Lz < 6, tau <= 0.5, g < 0, wall_kind != 0, null / misaligned /
- * undersized buffers, no sm_100 device.  *out is set to NULL on failure. */
+/* Creates a handle. Errors: Lx < 7, Lz < 6, tau <= 0.5, g < 0, wall_kind not 0/1, wall temperatures <= 0 with
+ * wall_kind 1, null pop_buf0 / misaligned / undersized buffers, no sm_100 device.  *out is set to NULL on failure. */
 int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p);
+
+/* ---- z-slabs: the lattice split along z over several handles (one per GPU), SURVEY 8(f)4.  The paper splits
+ * along x over N_p GPUs and hides the halo exchange behind the bulk propagate on separate streams (PAPER.md:110,
+ * 116-118, Fig. 3-4); with x-fastest storage the contiguous cut is along z.
+ * A slab owns rows [z0, z0+nz) of an Lx x Lz_global lattice and stores 3 ghost rows per open side (max |e_z| = 3).
+ * Dense arrays of every other call (fields [nz][Lx], populations [37][nz][Lx], row profiles [nz]) cover the OWN rows;
+ * lbm_totals and the widths of lbm_mixing_widths are the slab's partial sums (add them over the slabs).
+ * One time step of a slab, every step:
+ *   lbm_slab_pack(side)      my outermost own rows -> message (26 population-rows), per open side
+ *   lbm_slab_step(INTERIOR)  rows that read no ghost row; overlaps the exchange (another stream)
+ *   ... the caller moves the messages (cudaMemcpyAsync between devices, ncclSend/ncclRecv, ...) ...
+ *   lbm_slab_unpack(side)    neighbour's message -> my ghost rows of the CURRENT copy
+ *   lbm_slab_step(EDGES)     the remaining own rows; then the other copy becomes current.
+ * Results are bit-identical to the whole-lattice run.  Slabs use the one-step kernel and two lattice copies;
+ * lbm_step / lbm_run_host return LBM_ERR_INVALID for them.  lbm_init_rt fills ghost rows too (closed form);
+ * after lbm_init_equilibrium / lbm_set_populations the first exchange does. */
+#define LBM_SLAB_INTERIOR 0
+#define LBM_SLAB_EDGES 1
+size_t lbm_slab_buffer_bytes(int Lx, int Lz_global, int z0, int nz);   /* 0 if invalid (nz >= 6 rows inside the lattice) */
+int lbm_create_slab(lbm_t **out, int Lx, int Lz_global, int z0, int nz, const lbm_params *p);
+/* HOST outputs, any may be NULL: own row range, whether the sides are open (1) or walls (0), doubles per message. */
+int lbm_slab_info(const lbm_t *h, int *z0, int *nz, int *open_below, int *open_above, size_t *message_doubles);
+/* side 0 = towards lower z, 1 = towards higher z; msg_dev: DEVICE buffer of message_doubles doubles; asynchronous.
+ * LBM_ERR_INVALID if that side is a wall. */
+int lbm_slab_pack(lbm_t *h, int side, double *msg_dev, void *stream);
+int lbm_slab_unpack(lbm_t *h, int side, const double *msg_dev, void *stream);
+int lbm_slab_step(lbm_t *h, int part, void *stream);
 
 /* Frees the handle and its scratch; never the population buffers. NULL is a no-op. */
 int lbm_destroy(lbm_t *h);
@@ -96,11 +133,17 @@ int lbm_set_populations_host(lbm_t *h, const double *f_host, void *stream);
 int lbm_get_populations_host(lbm_t *h, double *f_host, void *stream);
 
 /* Enqueues n x (propagate + bc + collide) on `stream`; asynchronous.  Afterwards the
- * current lattice is the post-collision state of step n. */
+ * current lattice is the post-collision state of step n.
+ * Stream capture: the call only enqueues kernels, so it may be captured into a CUDA graph, but the handle's
+ * bookkeeping (which lattice copy is current, lbm_steps_done) advances when the call is made, not when the graph
+ * is replayed.  A captured sequence must therefore return to the same copy: LBM_ERR_INVALID if the n steps are
+ * an odd number of launches here (lbm_get_plan tells whether launches advance one or two steps); no other lbm_*
+ * call on the handle may be interleaved with replays; lbm_steps_done does not count replays. */
 int lbm_step(lbm_t *h, int n, void *stream);
 
 /* Hydrodynamic fields of the stored state (reading 8): rho, u^(H) = u - g_vec/2,
- * T^(H) = T + g^2/8, each a device pointer [Lz][Lx] or NULL to skip.  Asynchronous. */
+ * T^(H) = T + g^2/8, each a device pointer [Lz][Lx] or NULL to skip (LBM_ERR_INVALID if all four are NULL).
+ * Asynchronous. */
 int lbm_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *stream);
 
 /* Mixing widths of eq. 12 from the x-averaged T^(H), in sites, with the
@@ -126,6 +169,17 @@ int lbm_growth_rate(int n, const double *t, const double *L, double g, double At
  * reduction). Synchronises `stream`. */
 int lbm_totals(lbm_t *h, double *out4, void *stream);
 
+/* All of the above diagnostics in ONE pass over the lattice (lbm_mixing_widths, lbm_profiles and lbm_totals are
+ * calls of it): widths2 = {L_u, L_d} (eq. 12, needs distinct layer temperatures), totals4, and the row profiles
+ * Tbar, Trms, Ekbar, Ekrms [Lz].  HOST outputs, any may be NULL; the squared-deviation pass runs only if Trms or
+ * Ekrms is asked for.  Synchronises `stream`. */
+int lbm_diagnostics(lbm_t *h, double T_d, double T_m, double T_u, double *widths2, double *totals4, double *Tbar,
+                    double *Trms, double *Ekbar, double *Ekrms, void *stream);
+
+/* Scales of a Rayleigh-Taylor run (host arithmetic): Atwood number At = (T_d - T_u)/(T_d + T_u) (Table II,
+ * PAPER.md:144) and tau_RT = sqrt(Lx / (g At)), Lx in sites.  HOST outputs, any may be NULL. */
+int lbm_rt_scales(double Lx, double g, double T_d, double T_u, double *At, double *tau_rt);
+
 /* Host-buffer convenience used by the end-to-end benchmark: uploads kinetic fields (HOST, [Lz][Lx]),
  * initialises at equilibrium, runs n steps, downloads rho, u^(H), T^(H) (HOST, [Lz][Lx], any may be NULL).
  * Uses the handle's staging buffers (allocated on first use, 4 x Lx x Lz doubles). Synchronous. */
@@ -146,6 +200,11 @@ int lbm_fp64_peak(double *tflops, int iters, void *stream);
  * bit-identical results. */
 int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel (>= 3), or 0 = automatic */
+/* The launch plan lbm_step uses for this lattice with the current variant / zchunk settings (HOST outputs, any may
+ * be NULL): *fused = 1 if a launch advances two time steps (two-step kernel), 0 if one; *strip_width = columns per
+ * block of the two-step kernel (strip s covers columns [s w, (s+1) w)); *zchunk = rows per block (chunk c covers
+ * rows [c ZC, (c+1) ZC)).  Automatic choice: DESIGN.md section 6 (whole waves of blocks, few chunks). */
+int lbm_get_plan(lbm_t *h, int *fused, int *strip_width, int *zchunk);
 /* D2Q37 tables as the library uses them (host outputs, any may be NULL): e_x[37], e_z[37], w[37], r. */
 int lbm_tables(int *ex, int *ez, double *w, double *r);
 const char *lbm_last_error(void);

@@ -11,11 +11,23 @@ import ctypes as C
 from . import binding
 from .binding import LbmError, NPOP, lbm_params, lbm_rt_init
 
-__all__ = ["Lattice", "LbmError", "NPOP", "buffer_bytes", "tables", "growth_rate"]
+__all__ = ["Lattice", "Slab", "LbmError", "NPOP", "buffer_bytes", "slab_buffer_bytes", "tables", "growth_rate",
+           "rt_scales", "fp64_peak"]
 
 
 def buffer_bytes(Lx: int, Lz: int) -> int:
     return int(binding.load().lbm_buffer_bytes(Lx, Lz))
+
+
+def slab_buffer_bytes(Lx: int, Lz_global: int, z0: int, nz: int) -> int:
+    return int(binding.load().lbm_slab_buffer_bytes(Lx, Lz_global, z0, nz))
+
+
+def rt_scales(Lx: float, g: float, T_d: float, T_u: float):
+    """(At, tau_RT) of a Rayleigh-Taylor run (lbm_rt_scales: Table II / PAPER.md:126 arithmetic, in the library)."""
+    at, tr = C.c_double(), C.c_double()
+    binding.check(binding.load().lbm_rt_scales(Lx, g, T_d, T_u, C.byref(at), C.byref(tr)))
+    return at.value, tr.value
 
 
 def tables():
@@ -42,10 +54,23 @@ def fp64_peak(iters: int = 0, stream=None) -> float:
     return out.value
 
 
-def _stream_ptr(stream):
+def _stream_ptr(stream, device=None):
     import torch
-    s = stream if stream is not None else torch.cuda.current_stream()
+    s = stream if stream is not None else torch.cuda.current_stream(device)
     return C.c_void_p(s.cuda_stream)
+
+
+def _on_device(method):
+    """Runs a Lattice method with the lattice's device current (lbm_create binds the handle to the current device,
+    and every lbm_* call checks it)."""
+    import functools
+
+    @functools.wraps(method)
+    def wrapper(self, *args, **kwargs):
+        import torch
+        with torch.cuda.device(self.device):
+            return method(self, *args, **kwargs)
+    return wrapper
 
 
 def _dptr(t):
@@ -53,23 +78,32 @@ def _dptr(t):
 
 
 class Lattice:
-    """One Lx x Lz lattice resident on the current CUDA device (lbm_create)."""
+    """One Lx x Lz lattice resident on a CUDA device (lbm_create).  wall_kind 1: isothermal no-slip walls at
+    T_wall = (bottom, top).  inplace = True: one lattice copy instead of two (in-place streaming)."""
 
-    def __init__(self, Lx: int, Lz: int, tau: float, g: float, wall_kind: int = 0, device="cuda"):
+    def __init__(self, Lx: int, Lz: int, tau: float, g: float, wall_kind: int = 0, T_wall=(1.0, 1.0),
+                 inplace: bool = False, device="cuda", _slab=None):
         import torch
         self._lib = binding.load()
         if not torch.cuda.is_available():
             raise LbmError("no CUDA device: the lattice update has no CPU fallback")
         self.Lx, self.Lz, self.tau, self.g = int(Lx), int(Lz), float(tau), float(g)
         self.device = torch.device(device)
-        nbytes = buffer_bytes(Lx, Lz)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
+        nbytes = buffer_bytes(Lx, Lz) if _slab is None else slab_buffer_bytes(Lx, *_slab)
         if nbytes == 0:
-            raise LbmError(f"invalid lattice {Lx} x {Lz}")
-        # the two lattice copies (prv / nxt): torch owns the memory, the library only uses it
-        self._bufs = [torch.empty(nbytes // 8, dtype=torch.float64, device=self.device) for _ in range(2)]
-        p = lbm_params(tau, g, wall_kind, self._bufs[0].data_ptr(), self._bufs[1].data_ptr(), nbytes)
+            raise LbmError(f"invalid lattice {Lx} x {Lz}" + (f" / slab {_slab}" if _slab else ""))
+        # the lattice copies (prv / nxt, or the one copy of the in-place path): torch owns the memory
+        self._bufs = [torch.empty(nbytes // 8, dtype=torch.float64, device=self.device) for _ in range(1 if inplace else 2)]
+        p = lbm_params(tau, g, wall_kind, self._bufs[0].data_ptr(), None if inplace else self._bufs[1].data_ptr(), nbytes,
+                       float(T_wall[0]), float(T_wall[1]))
         h = C.c_void_p()
-        binding.check(self._lib.lbm_create(C.byref(h), Lx, Lz, C.byref(p)))
+        with torch.cuda.device(self.device):
+            if _slab is None:
+                binding.check(self._lib.lbm_create(C.byref(h), Lx, Lz, C.byref(p)))
+            else:
+                binding.check(self._lib.lbm_create_slab(C.byref(h), Lx, *_slab, C.byref(p)))
         self._h = h
 
     def close(self):
@@ -85,65 +119,94 @@ class Lattice:
             pass
 
     # ---- initial states
+    @_on_device
     def init_rt(self, seed: int, T_d, T_m, T_u, rho_m=1.0, delta=0.0, smooth_w=2.5, pert_kind=0, n_modes=0,
                 amp_lo=0.0, amp_hi=0.0, stream=None):
         ic = lbm_rt_init(T_d, T_m, T_u, rho_m, delta, smooth_w, pert_kind, n_modes, amp_lo, amp_hi)
-        binding.check(self._lib.lbm_init_rt(self._h, C.c_uint64(seed), C.byref(ic), _stream_ptr(stream)))
+        binding.check(self._lib.lbm_init_rt(self._h, C.c_uint64(seed), C.byref(ic), _stream_ptr(stream, self.device)))
 
+    @_on_device
     def init_equilibrium(self, rho, ux, uz, T, stream=None):
         self._check_fields(rho, ux, uz, T)
         binding.check(self._lib.lbm_init_equilibrium(self._h, _dptr(rho), _dptr(ux), _dptr(uz), _dptr(T),
-                                                     _stream_ptr(stream)))
+                                                     _stream_ptr(stream, self.device)))
 
     # ---- populations, canonical dense [37][Lz][Lx]
+    @_on_device
     def set_populations(self, f, stream=None):
         self._check_pops(f)
         fn = self._lib.lbm_set_populations if f.is_cuda else self._lib.lbm_set_populations_host
-        binding.check(fn(self._h, _dptr(f), _stream_ptr(stream)))
+        binding.check(fn(self._h, _dptr(f), _stream_ptr(stream, self.device)))
 
+    @_on_device
     def get_populations(self, out=None, host=False, stream=None):
         import torch
         if out is None:
             out = torch.empty((NPOP, self.Lz, self.Lx), dtype=torch.float64, device="cpu" if host else self.device)
         self._check_pops(out)
         fn = self._lib.lbm_get_populations if out.is_cuda else self._lib.lbm_get_populations_host
-        binding.check(fn(self._h, _dptr(out), _stream_ptr(stream)))
+        binding.check(fn(self._h, _dptr(out), _stream_ptr(stream, self.device)))
         return out
 
     # ---- the hot path
+    @_on_device
     def step(self, n: int = 1, stream=None):
-        binding.check(self._lib.lbm_step(self._h, int(n), _stream_ptr(stream)))
+        binding.check(self._lib.lbm_step(self._h, int(n), _stream_ptr(stream, self.device)))
 
     # ---- diagnostics
+    @_on_device
     def moments(self, rho=None, ux=None, uz=None, T=None, stream=None, alloc=True):
         import torch
         if alloc and rho is None and ux is None and uz is None and T is None:
             rho, ux, uz, T = (torch.empty((self.Lz, self.Lx), dtype=torch.float64, device=self.device) for _ in range(4))
         self._check_fields(*[x for x in (rho, ux, uz, T) if x is not None])
-        binding.check(self._lib.lbm_moments(self._h, _dptr(rho), _dptr(ux), _dptr(uz), _dptr(T), _stream_ptr(stream)))
+        binding.check(self._lib.lbm_moments(self._h, _dptr(rho), _dptr(ux), _dptr(uz), _dptr(T), _stream_ptr(stream, self.device)))
         return rho, ux, uz, T
 
+    @_on_device
     def mixing_widths(self, T_d, T_m, T_u, want_tbar=True, stream=None):
         import numpy as np
         lu, ld = C.c_double(), C.c_double()
         tbar = np.empty(self.Lz) if want_tbar else None
         binding.check(self._lib.lbm_mixing_widths(self._h, T_d, T_m, T_u, C.byref(lu), C.byref(ld),
-                                                  tbar.ctypes.data if want_tbar else None, _stream_ptr(stream)))
+                                                  tbar.ctypes.data if want_tbar else None, _stream_ptr(stream, self.device)))
         return lu.value, ld.value, tbar
 
+    @_on_device
     def profiles(self, stream=None):
         """(Tbar, Trms, Ekbar, Ekrms), host numpy arrays [Lz] (lbm_profiles)."""
         import numpy as np
         outs = [np.empty(self.Lz) for _ in range(4)]
-        binding.check(self._lib.lbm_profiles(self._h, *[o.ctypes.data for o in outs], _stream_ptr(stream)))
+        binding.check(self._lib.lbm_profiles(self._h, *[o.ctypes.data for o in outs], _stream_ptr(stream, self.device)))
         return tuple(outs)
 
+    @_on_device
+    def diagnostics(self, T_d=0.0, T_m=0.0, T_u=0.0, widths=True, totals=True, profiles=True, rms=True, stream=None):
+        """lbm_diagnostics: widths (L_u, L_d), lattice totals and row profiles in one pass over the lattice.
+        Returns a dict with the requested entries."""
+        import numpy as np
+        w, t = (C.c_double * 2)(), (C.c_double * 4)()
+        rows = [np.empty(self.Lz) if profiles and (rms or j % 2 == 0) else None for j in range(4)]
+        binding.check(self._lib.lbm_diagnostics(
+            self._h, T_d, T_m, T_u, w if widths else None, t if totals else None,
+            *[r.ctypes.data if r is not None else None for r in rows], _stream_ptr(stream, self.device)))
+        out = {}
+        if widths:
+            out["L_u"], out["L_d"] = w[0], w[1]
+        if totals:
+            out["totals"] = np.array(list(t))
+        if profiles:
+            out["Tbar"], out["Trms"], out["Ekbar"], out["Ekrms"] = rows
+        return out
+
+    @_on_device
     def totals(self, stream=None):
         import numpy as np
         out = (C.c_double * 4)()
-        binding.check(self._lib.lbm_totals(self._h, out, _stream_ptr(stream)))
+        binding.check(self._lib.lbm_totals(self._h, out, _stream_ptr(stream, self.device)))
         return np.array(list(out))
 
+    @_on_device
     def run_host(self, rho, ux, uz, T, n, outs=None, stream=None):
         """lbm_run_host: HOST (ideally pinned) kinetic fields in, n steps, HOST hydrodynamic fields out."""
         import torch
@@ -154,7 +217,7 @@ class Lattice:
         if outs is None:
             outs = tuple(torch.empty((self.Lz, self.Lx), dtype=torch.float64).pin_memory() for _ in range(4))
         binding.check(self._lib.lbm_run_host(self._h, *[_dptr(x) for x in ins], int(n), *[_dptr(x) for x in outs],
-                                             _stream_ptr(stream)))
+                                             _stream_ptr(stream, self.device)))
         return outs
 
     # ---- introspection
@@ -181,6 +244,12 @@ class Lattice:
     def set_zchunk(self, rows: int):
         binding.check(self._lib.lbm_set_zchunk(self._h, int(rows)))
 
+    def plan(self):
+        """(fused, strip_width, zchunk) of lbm_get_plan: how lbm_step launches on this lattice."""
+        f, w, z = C.c_int(), C.c_int(), C.c_int()
+        binding.check(self._lib.lbm_get_plan(self._h, C.byref(f), C.byref(w), C.byref(z)))
+        return bool(f.value), w.value, z.value
+
     # ---- argument checks (marshalling only)
     def _check_fields(self, *fields):
         import torch
@@ -192,3 +261,37 @@ class Lattice:
         import torch
         if f.dtype != torch.float64 or not f.is_contiguous() or f.numel() != NPOP * self.Lx * self.Lz:
             raise LbmError("populations must be a contiguous float64 tensor [37][Lz][Lx]")
+
+
+class Slab(Lattice):
+    """Rows [z0, z0 + nz) of an Lx x Lz_global lattice with ghost rows towards its neighbours (lbm_create_slab).
+    Dense arrays cover the slab's own rows ([nz][Lx], [37][nz][Lx]).  One step = pack -> step(INTERIOR) ->
+    (the caller moves the messages) -> unpack -> step(EDGES); `exchange_and_step` does it for slabs on one device."""
+    INTERIOR, EDGES = 0, 1
+
+    def __init__(self, Lx: int, Lz_global: int, z0: int, nz: int, tau: float, g: float, wall_kind: int = 0,
+                 T_wall=(1.0, 1.0), device="cuda"):
+        super().__init__(Lx, nz, tau, g, wall_kind=wall_kind, T_wall=T_wall, device=device, _slab=(Lz_global, z0, nz))
+        self.Lz_global, self.z0, self.nz = int(Lz_global), int(z0), int(nz)
+        z, n, lo, hi, m = C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_size_t()
+        binding.check(self._lib.lbm_slab_info(self._h, C.byref(z), C.byref(n), C.byref(lo), C.byref(hi), C.byref(m)))
+        self.open_below, self.open_above, self.message_doubles = bool(lo.value), bool(hi.value), int(m.value)
+
+    def new_message(self):
+        import torch
+        return torch.empty(self.message_doubles, dtype=torch.float64, device=self.device)
+
+    @_on_device
+    def pack(self, side: int, msg, stream=None):
+        binding.check(self._lib.lbm_slab_pack(self._h, int(side), _dptr(msg), _stream_ptr(stream, self.device)))
+
+    @_on_device
+    def unpack(self, side: int, msg, stream=None):
+        binding.check(self._lib.lbm_slab_unpack(self._h, int(side), _dptr(msg), _stream_ptr(stream, self.device)))
+
+    @_on_device
+    def step_part(self, part: int, stream=None):
+        binding.check(self._lib.lbm_slab_step(self._h, int(part), _stream_ptr(stream, self.device)))
+
+    def step(self, n: int = 1, stream=None):
+        raise LbmError("a slab is stepped with pack / step_part / unpack (its ghost rows are exchanged every step)")

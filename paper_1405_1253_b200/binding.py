@@ -18,7 +18,9 @@ SYMBOLS = [
     "lbm_buffer_bytes", "lbm_create", "lbm_destroy", "lbm_init_rt", "lbm_init_equilibrium",
     "lbm_set_populations", "lbm_get_populations", "lbm_set_populations_host", "lbm_get_populations_host",
     "lbm_step", "lbm_moments", "lbm_mixing_widths", "lbm_profiles", "lbm_growth_rate", "lbm_totals", "lbm_run_host", "lbm_steps_done",
-    "lbm_layout", "lbm_kernel_launches", "lbm_fp64_peak", "lbm_set_variant", "lbm_set_zchunk", "lbm_tables", "lbm_last_error",
+    "lbm_layout", "lbm_kernel_launches", "lbm_fp64_peak", "lbm_set_variant", "lbm_set_zchunk", "lbm_get_plan", "lbm_tables", "lbm_last_error",
+    "lbm_diagnostics", "lbm_rt_scales", "lbm_slab_buffer_bytes", "lbm_create_slab", "lbm_slab_info", "lbm_slab_pack",
+    "lbm_slab_unpack", "lbm_slab_step",
 ]
 
 
@@ -28,7 +30,8 @@ class LbmError(RuntimeError):
 
 class lbm_params(C.Structure):
     _fields_ = [("tau", C.c_double), ("g", C.c_double), ("wall_kind", C.c_int), ("pop_buf0", C.c_void_p),
-                ("pop_buf1", C.c_void_p), ("buf_bytes", C.c_size_t)]
+                ("pop_buf1", C.c_void_p), ("buf_bytes", C.c_size_t), ("T_wall_bottom", C.c_double),
+                ("T_wall_top", C.c_double)]
 
 
 class lbm_rt_init(C.Structure):
@@ -72,9 +75,20 @@ def load():
     L.lbm_fp64_peak.argtypes = [dp, C.c_int, vp]
     L.lbm_set_variant.argtypes = [vp, C.c_int]
     L.lbm_set_zchunk.argtypes = [vp, C.c_int]
+    L.lbm_get_plan.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.lbm_tables.argtypes = [C.POINTER(C.c_int), C.POINTER(C.c_int), dp, dp]
+    L.lbm_diagnostics.argtypes = [vp, C.c_double, C.c_double, C.c_double, vp, vp, vp, vp, vp, vp, vp]
+    L.lbm_rt_scales.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, dp, dp]
+    L.lbm_slab_buffer_bytes.restype = C.c_size_t
+    L.lbm_slab_buffer_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int]
+    L.lbm_create_slab.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(lbm_params)]
+    L.lbm_slab_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int),
+                                C.POINTER(C.c_size_t)]
+    L.lbm_slab_pack.argtypes = [vp, C.c_int, vp, vp]
+    L.lbm_slab_unpack.argtypes = [vp, C.c_int, vp, vp]
+    L.lbm_slab_step.argtypes = [vp, C.c_int, vp]
     for name in SYMBOLS:
-        if name not in ("lbm_buffer_bytes", "lbm_last_error"):
+        if name not in ("lbm_buffer_bytes", "lbm_slab_buffer_bytes", "lbm_last_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L

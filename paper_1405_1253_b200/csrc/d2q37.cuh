@@ -254,6 +254,18 @@ __device__ __forceinline__ void equilibrium_blend(const double (&fin)[NPOP], dou
                                  [&](auto L, double v) { out[decltype(L)::value] = v; }, keep, scale, ux, uz, T);
 }
 
+// Isothermal no-slip wall rows (reading 19; "bc ... adjusts population values at sites with
+// coordinates z = 0, 1, 2 and z = Lz-3, Lz-2, Lz-1"): the equilibrium part of the post-propagate populations is moved
+// to the wall state, density and non-equilibrium part kept,
+//   f <- f - f_eq(rho*, u*, T*) + f_eq(rho*, u_w, T_w),   u_w = (0, g/2),  T_w = T_wall - g^2/8,
+// the kinetic moments that PAPER.md:94 maps to u^(H) = 0, T^(H) = T_wall.  The collision then runs unchanged.
+__device__ __forceinline__ void wall_adjust(double (&f)[NPOP], double uwz, double Tw)
+{
+    const Kinetic k = kinetic_moments(f);
+    equilibrium_blend<true>(f, f, 1.0, -k.rho, k.ux, k.uz, k.T);
+    equilibrium_blend<true>(f, f, 1.0, k.rho, 0.0, uwz, Tw);
+}
+
 // One collision: moments of the post-propagate populations, equilibrium shifted by
 // u' = u + g_vec tau = (u_x, u_z - g tau), T' = T + tau (dt - tau) g^2 / d, BGK relaxation.
 //   omega = dt/tau, gtau = g tau, dT = tau (1 - tau) g^2 / 2.

@@ -1,6 +1,6 @@
 // lbm_api.cu -- the C ABI declared in include/lbm.h: handle, argument checks, kernel launches.
-// Every arithmetic step of the path runs in the kernels of lbm_step.cuh / lbm_aux.cuh; this file only
-// validates, draws the interface perturbation (host, O(Lx)), launches and copies.
+// Every arithmetic step of the path runs in the kernels of lbm_step.cuh / lbm_step2s.cuh / lbm_aux.cuh; this file
+// only validates, draws the interface perturbation (host, O(Lx)), plans launches, launches and copies.
 #include <cuda.h>
 #include <cuda_runtime.h>
 
@@ -37,9 +37,11 @@ int fail(int code, const char *fmt, ...)
 
 constexpr int ROW_ALIGN = 16;     // doubles: rows start on 128-byte lines
 constexpr int PLANE_PAD = 272;    // doubles (17 x 128 B): keeps the 37 plane bases off a power-of-two stride
+constexpr int GHOST = 3;          // ghost rows per open side of a z-slab (max |e_z|)
 
-int pitch_of(int Lx) { return (Lx + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN; }
-long long plane_of(int Lx, int Lz) { return (long long)pitch_of(Lx) * Lz + PLANE_PAD; }
+// row = [XH spare | Lx sites | XH spare], padded to 128 bytes
+int pitch_of(int Lx) { return (Lx + 2 * lbm::XH + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN; }
+long long plane_of(int Lx, int rows) { return (long long)pitch_of(Lx) * rows + PLANE_PAD; }
 
 // SplitMix64 (reading 12); U = (x >> 11) 2^-53
 struct SplitMix {
@@ -70,10 +72,11 @@ void draw_interface(SplitMix &rng, const lbm_rt_init &ic, int Lx, std::vector<do
     }
 }
 
-// Tensor maps for the TMA loads of the warp-specialised two-step kernel (lbm_step2s.cuh): the lattice copy `buf`
-// as a rank-3 tensor (x: Lx, z: Lz, l: 37) with strides (pitch, plane), box (SP, R, n) for n = 3, 5, 7.
+// Tensor maps for the TMA loads of the warp-specialised two-step kernel (lbm_step2s.cuh): the lattice copy as a
+// rank-3 tensor (x: XH + Lx + XH stored columns, z: Lz, l: 37) with strides (pitch, plane), box (SP, R, n) for
+// n = 3, 5, 7.  `ubuf` is the start of the allocation (stored column -XH of row 0).
 // cuTensorMapEncodeTiled is fetched through the runtime (no link-time dependency on libcuda).
-bool encode_step2s_maps(const double *buf, int Lx, int Lz, int pitch, long long plane, lbm::Step2sMaps &out)
+bool encode_step2s_maps(const double *ubuf, int Lx, int Lz, int pitch, long long plane, lbm::Step2sMaps &out)
 {
     using S = lbm::Step2sWide;
     typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -91,11 +94,11 @@ bool encode_step2s_maps(const double *buf, int Lx, int Lz, int pitch, long long 
     }
     static_assert(sizeof(CUtensorMap) == 128, "Step2sMaps holds three 128-byte tensor maps");
     for (int i = 0; i < 3; ++i) {
-        const cuuint64_t dims[3] = {(cuuint64_t)Lx, (cuuint64_t)Lz, (cuuint64_t)LBM_NPOP};
+        const cuuint64_t dims[3] = {(cuuint64_t)(Lx + 2 * lbm::XH), (cuuint64_t)Lz, (cuuint64_t)LBM_NPOP};
         const cuuint64_t strides[2] = {(cuuint64_t)pitch * 8, (cuuint64_t)plane * 8};
         const cuuint32_t box[3] = {(cuuint32_t)S::SP, (cuuint32_t)S::R, (cuuint32_t)(3 + 2 * i)};
         const cuuint32_t estr[3] = {1, 1, 1};
-        if (encode((CUtensorMap *)out.m[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)buf, dims, strides, box, estr,
+        if (encode((CUtensorMap *)out.m[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)ubuf, dims, strides, box, estr,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
             return false;
@@ -105,27 +108,271 @@ bool encode_step2s_maps(const double *buf, int Lx, int Lz, int pitch, long long 
 
 }  // namespace
 
+// launch plan of lbm_step (make_plan)
+struct lbm_plan {
+    bool valid, fused;
+    int w, strips, ZC, chunks;
+};
+
 struct lbm_handle {
-    int Lx, Lz, pitch;
+    int dev;               // CUDA device the handle was created on (every call must run with it current)
+    int Lx, Lz, pitch;     // Lz = STORED rows (a z-slab: its own rows plus ghost rows)
     long long plane;
     double tau, g;
-    double *buf[2];
+    int wall_kind;
+    double T_wall_lo, T_wall_hi;
+    double *ubuf[2];       // the caller's buffers
+    double *buf[2];        // site (0,0) of population 0 in each copy (ubuf + XH); buf[1] = null: in-place, one copy
+    bool inplace, layout_m;   // in-place path: layout_m after an odd number of steps (lbm_step.cuh)
+    bool wrap_ok[2];       // the wrap columns of copy i hold the periodic images of its current contents
+    // z-slab (lbm_create_slab): height of the whole lattice, first own global row, own rows, ghost rows below / above
+    bool slab;
+    int Lz_glob, z0, nz, glo, ghi;
+    int slab_phase;        // 0: ready for lbm_slab_step(INTERIOR), 1: interior launched, edges pending
     int cur;               // index of the current lattice
     long long steps, launches;
     int variant;
-    int zchunk;            // rows per block of the two-step kernel (multiple of 3; 0 = automatic)
+    int zchunk;            // rows per block of the two-step kernel (0 = automatic)
     int sm_count;
-    bool tma_ok;              // tensor maps of both lattice copies encoded (two-step kernel)
+    lbm_plan plan;         // cached; invalidated by lbm_set_variant / lbm_set_zchunk
+    bool tma_ok;           // tensor maps of both lattice copies encoded (two-step kernel)
     lbm::Step2sMaps maps[2];
-    double *scratch;       // device: Tbar[Lz] | row partials[4 Lz] | results[8] | h_lo[Lx] | h_hi[Lx]
+    double *scratch;       // device: row diagnostics [8][nz] | results[8] | h_lo[Lx] | h_hi[Lx]
     double *stage[4];      // device staging fields for lbm_run_host (lazy)
-    lbm::Layout layout() const { return lbm::Layout{Lx, Lz, pitch, plane}; }
-    double *d_tbar() const { return scratch; }
-    double *d_partial() const { return scratch + Lz; }
-    double *d_result() const { return scratch + 5LL * Lz; }
-    double *d_hlo() const { return scratch + 5LL * Lz + 8; }
-    double *d_hhi() const { return scratch + 5LL * Lz + 8 + Lx; }
+    double *plane_stage;   // device staging of one dense population plane for the _host copies of in-place handles (lazy)
+    lbm::Layout layout() const { return lbm::Layout{Lx, Lz, pitch, plane, glo, nz, layout_m}; }
+    double *d_rows() const { return scratch; }
+    double *d_result() const { return scratch + 8LL * nz; }
+    double *d_hlo() const { return scratch + 8LL * nz + 8; }
+    double *d_hhi() const { return scratch + 8LL * nz + 8 + Lx; }
+    bool wall_lo() const { return !slab || z0 == 0; }
+    bool wall_hi() const { return !slab || z0 + nz == Lz_glob; }
 };
+
+namespace {
+
+int check_handle(const lbm_t *h, const char *fn)
+{
+    if (!h) return fail(LBM_ERR_INVALID, "%s: null handle", fn);
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return fail(LBM_ERR_NODEVICE, "%s: no CUDA device", fn); }
+    if (dev != h->dev)
+        return fail(LBM_ERR_INVALID, "%s: the handle lives on device %d but device %d is current", fn, h->dev, dev);
+    return LBM_OK;
+}
+#define NEED(h) do { int rc_ = check_handle((h), __func__); if (rc_) return rc_; } while (0)
+#define NEED_HOST(h) do { if (!(h)) return fail(LBM_ERR_INVALID, "%s: null handle", __func__); } while (0)
+#define LAUNCHED(h) do { CUDA_TRY(cudaGetLastError()); (h)->launches++; } while (0)
+
+dim3 own_grid(const lbm_t *h, int tx) { return dim3((h->Lx + tx - 1) / tx, h->nz, 1); }
+
+lbm::StepArgs step_args(const lbm_t *h)
+{
+    lbm::StepArgs a;
+    a.Lx = h->Lx; a.Lz = h->Lz; a.pitch = h->pitch; a.plane = h->plane;
+    a.omega = 1.0 / h->tau;
+    a.gtau = h->g * h->tau;
+    a.dT = 0.5 * h->tau * (1.0 - h->tau) * h->g * h->g;
+    // wall_kind 1 (reading 19): kinetic wall state u_w = (0, g/2), T_w = T_wall - g^2/8 (PAPER.md:94 backwards)
+    a.iso_lo = h->wall_kind == 1 && h->wall_lo();
+    a.iso_hi = h->wall_kind == 1 && h->wall_hi();
+    a.uwz = 0.5 * h->g;
+    a.Tw_lo = h->T_wall_lo - 0.125 * h->g * h->g;
+    a.Tw_hi = h->T_wall_hi - 0.125 * h->g * h->g;
+    a.wrap_store = 0;
+    a.w = 0;
+    lbm::fill_offsets(a);
+    return a;
+}
+
+// Launch plan of lbm_step for this lattice.  The two-step kernel runs strips of w <= TX columns in chunks of ZC rows,
+// one block per SM at a time, every block (ZC + 6)/R passes of about the same duration: the plan minimises
+//   (waves + 0.3) x (ZC + 6 + fill),  waves = ceil(strips x chunks / SMs)
+// over the strip count and ZC (whole waves: no tail; few chunks: little warm-up -- a chunk recomputes the 6
+// intermediate rows below it; + 0.3: the blocks of a wave do not finish together -- wall chunks gather three rows
+// from global memory -- so a launch of few long waves waits for its slowest block), and takes the one-step kernel
+// where that is predicted to be faster (small lattices).  Measurements: profiles/r2_two_step.md.
+const lbm_plan &make_plan(lbm_t *h)
+{
+    using S2 = lbm::Step2sWide;
+    if (h->plan.valid) return h->plan;
+    lbm_plan &p = h->plan;
+    p = lbm_plan{};
+    const int Lx = h->Lx, Lz = h->Lz, sms = h->sm_count > 0 ? h->sm_count : 148;
+    const int ns_min = (Lx + S2::TX - 1) / S2::TX;
+    double best = 1e300;
+    for (int ns = ns_min; ns <= ns_min + ns_min / 4 + 1; ++ns) {
+        // strips start on 32-byte sectors (w a multiple of 4): consumer rows are whole sectors
+        int w = 4 * ((Lx + 4 * ns - 1) / (4 * ns));
+        if (w > S2::TX) continue;
+        if (w < 8) w = 8;
+        const int strips = (Lx + w - 1) / w;
+        for (int chunks = 1; chunks <= (Lz + 15) / 16; ++chunks) {
+            int ZC = (Lz + chunks - 1) / chunks;
+            ZC = (ZC + 1) / 2 * 2;                            // whole passes of R = 2 rows
+            if (ZC < 6) ZC = 6;
+            const int nch = (Lz + ZC - 1) / ZC;
+            const long long waves = ((long long)strips * nch + sms - 1) / sms;
+            const double cost = ((double)waves + 0.3) * (ZC + 6 + 4);   // + 4: pipeline fill of a block (first TMA round trip)
+            if (cost < best - 1e-9) { best = cost; p.w = w; p.strips = strips; p.ZC = ZC; p.chunks = nch; }
+        }
+    }
+    if (h->zchunk > 0) {                                      // rows per block forced (tests, experiments)
+        p.ZC = h->zchunk;
+        p.chunks = (Lz + p.ZC - 1) / p.ZC;
+        best = ((double)(((long long)p.strips * p.chunks + sms - 1) / sms) + 0.3) * (p.ZC + 10);
+    }
+    // predicted time of two steps, microseconds: the two-step kernel spends ~0.85 us per row of a chunk (1.7 us per
+    // pass of two rows) plus ~4 us per launch; the one-step kernel ~92 ps per site and step plus ~3 us per launch
+    // (profiles/r2_sweep.md)
+    const double t_fused = 0.85 * best + 4.0;
+    const double t_single = 2.0 * (92e-6 * (double)Lx * Lz + 3.0);
+    const bool can_fuse = h->tma_ok && !h->inplace && !h->slab;
+    p.fused = can_fuse && (h->variant == 3 || (h->variant == 0 && t_fused < t_single));
+    p.valid = true;
+    return p;
+}
+
+// periodic images for the two-step kernel's boxes (a1), if copy `i` was last written by anything but that kernel
+int refresh_wrap_columns(lbm_t *h, int i, cudaStream_t st)
+{
+    if (h->wrap_ok[i]) return LBM_OK;
+    lbm::wrap_columns_kernel<lbm::XW><<<h->Lz, 2 * lbm::XW * LBM_NPOP, 0, st>>>(h->buf[i], h->layout());
+    LAUNCHED(h);
+    h->wrap_ok[i] = true;
+    return LBM_OK;
+}
+
+template <bool ISO>
+int launch_one_step(lbm_t *h, const lbm::StepArgs &a, int k0, int k1, cudaStream_t st)
+{
+    if (k1 <= k0) return LBM_OK;
+    const int rows = k1 - k0;
+    if (h->inplace) {
+        // 128-thread blocks; even steps scatter back to the gathered slots, odd steps are local (lbm_step.cuh)
+        const dim3 grid((h->Lx + 127) / 128, rows);
+        if (!h->layout_m) lbm::step_inplace_even_kernel<128, ISO><<<grid, 128, 0, st>>>(a, k0, k1);
+        else lbm::step_inplace_odd_kernel<128, ISO><<<grid, 128, 0, st>>>(a, k0, k1);
+    } else if (h->variant == 2 || (h->variant == 0 && (long long)h->Lx * h->Lz < (1LL << 20))) {
+        // 128-thread blocks are a few per cent faster on the small (L2-resident, few-wave) lattices, 256 on the large
+        lbm::step_kernel_site<128, 1, ISO><<<dim3((h->Lx + 127) / 128, rows), dim3(128, 1), 0, st>>>(a, k0, k1);
+    } else {  // 256 threads = 2 blocks/SM at 128 registers: fastest one-step shape at 4096x8192
+        lbm::step_kernel_site<256, 1, ISO><<<dim3((h->Lx + 255) / 256, rows), dim3(256, 1), 0, st>>>(a, k0, k1);
+    }
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
+int one_step_rows(lbm_t *h, lbm::StepArgs &a, int k0, int k1, cudaStream_t st)
+{
+    a.src = h->buf[h->cur];
+    a.dst = h->inplace ? h->buf[h->cur] : h->buf[h->cur ^ 1];
+    return h->wall_kind == 1 ? launch_one_step<true>(h, a, k0, k1, st) : launch_one_step<false>(h, a, k0, k1, st);
+}
+
+// a5: after a step the other copy is current (two copies) or the layout has alternated (one copy)
+void advance(lbm_t *h, int nsteps)
+{
+    if (h->inplace) {
+        if (nsteps % 2) h->layout_m = !h->layout_m;
+    } else {
+        h->cur ^= 1;
+    }
+    h->steps += nsteps;
+}
+
+int create_common(lbm_t **out, int Lx, int rows_stored, const lbm_params *p, const char *fn)
+{
+    if (!out) return fail(LBM_ERR_INVALID, "%s: out is null", fn);
+    *out = nullptr;
+    if (!p) return fail(LBM_ERR_INVALID, "%s: params is null", fn);
+    // Lx >= 7 keeps the seven wrapped source columns of a site distinct (one wrap suffices); Lz >= 6
+    // keeps the three wall rows of the two walls disjoint (PAPER.md:114)
+    if (Lx < 7 || rows_stored < 6) return fail(LBM_ERR_INVALID, "%s: need Lx >= 7 and Lz >= 6 (got %d x %d)", fn, Lx, rows_stored);
+    if (rows_stored > 65535) return fail(LBM_ERR_INVALID, "%s: Lz <= 65535 (got %d)", fn, rows_stored);
+    if (!(p->tau > 0.5)) return fail(LBM_ERR_INVALID, "%s: tau must be > 0.5 (got %g)", fn, p->tau);
+    if (!(p->g >= 0.0)) return fail(LBM_ERR_INVALID, "%s: g must be >= 0 (got %g)", fn, p->g);
+    if (p->wall_kind != 0 && p->wall_kind != 1) return fail(LBM_ERR_INVALID, "%s: wall_kind %d not supported", fn, p->wall_kind);
+    if (p->wall_kind == 1 && !(p->T_wall_bottom > 0.0 && p->T_wall_top > 0.0))
+        return fail(LBM_ERR_INVALID, "%s: wall_kind 1 needs wall temperatures > 0 (got %g, %g)", fn, p->T_wall_bottom, p->T_wall_top);
+    if (!p->pop_buf0 || p->pop_buf0 == p->pop_buf1)
+        return fail(LBM_ERR_INVALID, "%s: pop_buf0 must be set and differ from pop_buf1", fn);
+    if (((uintptr_t)p->pop_buf0 | (uintptr_t)p->pop_buf1) & 255)
+        return fail(LBM_ERR_INVALID, "%s: population buffers must be 256-byte aligned", fn);
+    const size_t need = (size_t)plane_of(Lx, rows_stored) * LBM_NPOP * sizeof(double);
+    if (p->buf_bytes < need) return fail(LBM_ERR_INVALID, "%s: buffers have %zu bytes, need %zu", fn, p->buf_bytes, need);
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(LBM_ERR_NODEVICE, "%s: no CUDA device", fn);
+    }
+    if (prop.major != 10) return fail(LBM_ERR_NODEVICE, "%s: built for sm_100a, device is sm_%d%d", fn, prop.major, prop.minor);
+    lbm_handle *h = new (std::nothrow) lbm_handle();
+    if (!h) return fail(LBM_ERR_INVALID, "%s: out of host memory", fn);
+    h->dev = dev;
+    h->Lx = Lx; h->Lz = rows_stored; h->pitch = pitch_of(Lx); h->plane = plane_of(Lx, rows_stored);
+    h->tau = p->tau; h->g = p->g; h->sm_count = prop.multiProcessorCount;
+    h->wall_kind = p->wall_kind; h->T_wall_lo = p->T_wall_bottom; h->T_wall_hi = p->T_wall_top;
+    h->ubuf[0] = (double *)p->pop_buf0; h->ubuf[1] = (double *)p->pop_buf1;
+    h->buf[0] = h->ubuf[0] + lbm::XH;
+    h->buf[1] = h->ubuf[1] ? h->ubuf[1] + lbm::XH : nullptr;
+    h->inplace = h->ubuf[1] == nullptr; h->layout_m = false;
+    h->wrap_ok[0] = h->wrap_ok[1] = false;
+    h->slab = false; h->Lz_glob = rows_stored; h->z0 = 0; h->nz = rows_stored; h->glo = h->ghi = 0; h->slab_phase = 0;
+    h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 0; h->scratch = nullptr; h->plane_stage = nullptr;
+    h->plan = lbm_plan{};
+    h->tma_ok = false;
+    for (auto &s : h->stage) s = nullptr;
+    *out = h;
+    return LBM_OK;
+}
+
+int finish_create(lbm_t **out)
+{
+    lbm_handle *h = *out;
+    if (!h->inplace && !h->slab) {
+        h->tma_ok = encode_step2s_maps(h->ubuf[0], h->Lx, h->Lz, h->pitch, h->plane, h->maps[0]) &&
+                    encode_step2s_maps(h->ubuf[1], h->Lx, h->Lz, h->pitch, h->plane, h->maps[1]);
+        // the opt-in to > 48 KB of dynamic shared memory is per device (context), so it is made for every handle
+        using S2 = lbm::Step2sWide;
+        if (h->tma_ok && (cudaFuncSetAttribute(lbm::step2s_kernel<S2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2::SMEM) != cudaSuccess ||
+                          cudaFuncSetAttribute(lbm::step2s_kernel<S2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2::SMEM) != cudaSuccess)) {
+            cudaGetLastError();
+            h->tma_ok = false;
+        }
+    }
+    cudaError_t e = cudaMalloc(&h->scratch, sizeof(double) * (8LL * h->nz + 8 + 2LL * h->Lx));
+    if (e != cudaSuccess) {
+        delete h;
+        *out = nullptr;
+        return fail(LBM_ERR_CUDA, "lbm_create: cudaMalloc scratch: %s", cudaGetErrorString(e));
+    }
+    return LBM_OK;
+}
+
+// the 26 (row, population) pairs of a slab message; `send`: the own rows the neighbour on `side` needs, else the
+// ghost rows on `side` that the neighbour's message fills
+lbm::SlabRows slab_rows(const lbm_t *h, int side, bool send)
+{
+    lbm::SlabRows s;
+    int j = 0;
+    for (int d = 1; d <= GHOST; ++d) {
+        // side 1 (above): the upper neighbour's ghost row at distance d below its first row is my own row nz - d;
+        // it is read by its rows 0 .. 3-d with e_z >= d.  side 0 (below): mirror image, e_z <= -d.
+        int row;
+        if (send) row = side == 1 ? h->glo + h->nz - d : h->glo + d - 1;
+        else row = side == 1 ? h->glo + h->nz + d - 1 : h->glo - d;
+        for (int l = 0; l < LBM_NPOP; ++l) {
+            const int ez = d2q37::pop_ez(l);
+            const bool wanted = send ? (side == 1 ? ez >= d : ez <= -d) : (side == 1 ? ez <= -d : ez >= d);
+            if (wanted) { s.row[j] = row; s.l[j] = l; ++j; }
+        }
+    }
+    return s;  // j == 26
+}
+
+}  // namespace
 
 extern "C" {
 
@@ -135,6 +382,13 @@ size_t lbm_buffer_bytes(int Lx, int Lz)
 {
     if (Lx < 7 || Lz < 6) return 0;
     return (size_t)plane_of(Lx, Lz) * LBM_NPOP * sizeof(double);
+}
+
+size_t lbm_slab_buffer_bytes(int Lx, int Lz_global, int z0, int nz)
+{
+    if (Lx < 7 || Lz_global < 6 || z0 < 0 || nz < GHOST || z0 + nz > Lz_global) return 0;
+    const int rows = nz + (z0 > 0 ? GHOST : 0) + (z0 + nz < Lz_global ? GHOST : 0);
+    return rows < 6 ? 0 : (size_t)plane_of(Lx, rows) * LBM_NPOP * sizeof(double);
 }
 
 int lbm_tables(int *ex, int *ez, double *w, double *r)
@@ -150,57 +404,35 @@ int lbm_tables(int *ex, int *ez, double *w, double *r)
 
 int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p)
 {
-    if (!out) return fail(LBM_ERR_INVALID, "lbm_create: out is null");
-    *out = nullptr;
-    if (!p) return fail(LBM_ERR_INVALID, "lbm_create: params is null");
-    // Lx >= 7 keeps the seven wrapped source columns of a site distinct (one wrap suffices); Lz >= 6
-    // keeps the three wall rows of the two walls disjoint (PAPER.md:114)
-    if (Lx < 7 || Lz < 6) return fail(LBM_ERR_INVALID, "lbm_create: need Lx >= 7 and Lz >= 6 (got %d x %d)", Lx, Lz);
-    if (Lz > 65535) return fail(LBM_ERR_INVALID, "lbm_create: Lz <= 65535 (got %d)", Lz);
-    if (!(p->tau > 0.5)) return fail(LBM_ERR_INVALID, "lbm_create: tau must be > 0.5 (got %g)", p->tau);
-    if (!(p->g >= 0.0)) return fail(LBM_ERR_INVALID, "lbm_create: g must be >= 0 (got %g)", p->g);
-    if (p->wall_kind != 0) return fail(LBM_ERR_INVALID, "lbm_create: wall_kind %d not supported", p->wall_kind);
-    if (!p->pop_buf0 || !p->pop_buf1 || p->pop_buf0 == p->pop_buf1)
-        return fail(LBM_ERR_INVALID, "lbm_create: two distinct population buffers are required");
-    if (((uintptr_t)p->pop_buf0 | (uintptr_t)p->pop_buf1) & 255)
-        return fail(LBM_ERR_INVALID, "lbm_create: population buffers must be 256-byte aligned");
-    if (p->buf_bytes < lbm_buffer_bytes(Lx, Lz))
-        return fail(LBM_ERR_INVALID, "lbm_create: buffers have %zu bytes, need %zu", p->buf_bytes, lbm_buffer_bytes(Lx, Lz));
-    int dev = 0;
-    cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-        cudaGetLastError();
-        return fail(LBM_ERR_NODEVICE, "lbm_create: no CUDA device");
-    }
-    if (prop.major != 10) return fail(LBM_ERR_NODEVICE, "lbm_create: built for sm_100a, device is sm_%d%d", prop.major, prop.minor);
-    lbm_handle *h = new (std::nothrow) lbm_handle();
-    if (!h) return fail(LBM_ERR_INVALID, "lbm_create: out of host memory");
-    h->Lx = Lx; h->Lz = Lz; h->pitch = pitch_of(Lx); h->plane = plane_of(Lx, Lz);
-    h->tau = p->tau; h->g = p->g; h->sm_count = prop.multiProcessorCount;
-    h->buf[0] = (double *)p->pop_buf0; h->buf[1] = (double *)p->pop_buf1;
-    h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 0; h->scratch = nullptr;
-    h->tma_ok = encode_step2s_maps(h->buf[0], Lx, Lz, h->pitch, h->plane, h->maps[0]) &&
-                encode_step2s_maps(h->buf[1], Lx, Lz, h->pitch, h->plane, h->maps[1]);
-    for (auto &s : h->stage) s = nullptr;
-    cudaError_t e = cudaMalloc(&h->scratch, sizeof(double) * (5LL * Lz + 8 + 2LL * Lx));
-    if (e != cudaSuccess) { delete h; return fail(LBM_ERR_CUDA, "lbm_create: cudaMalloc scratch: %s", cudaGetErrorString(e)); }
-    *out = h;
-    return LBM_OK;
+    int rc = create_common(out, Lx, Lz, p, "lbm_create");
+    if (rc) return rc;
+    return finish_create(out);
+}
+
+int lbm_create_slab(lbm_t **out, int Lx, int Lz_global, int z0, int nz, const lbm_params *p)
+{
+    if (out) *out = nullptr;
+    if (Lz_global < 6 || z0 < 0 || nz < 2 * GHOST || z0 + nz > Lz_global)
+        return fail(LBM_ERR_INVALID, "lbm_create_slab: rows [%d, %d) of %d: a slab needs >= %d rows inside the lattice",
+                    z0, z0 + nz, Lz_global, 2 * GHOST);
+    if (p && !p->pop_buf1) return fail(LBM_ERR_INVALID, "lbm_create_slab: a slab needs two lattice copies");
+    const int glo = z0 > 0 ? GHOST : 0, ghi = z0 + nz < Lz_global ? GHOST : 0;
+    int rc = create_common(out, Lx, glo + nz + ghi, p, "lbm_create_slab");
+    if (rc) return rc;
+    lbm_handle *h = *out;
+    h->slab = true; h->Lz_glob = Lz_global; h->z0 = z0; h->nz = nz; h->glo = glo; h->ghi = ghi;
+    return finish_create(out);
 }
 
 int lbm_destroy(lbm_t *h)
 {
     if (!h) return LBM_OK;
     cudaFree(h->scratch);
+    cudaFree(h->plane_stage);
     for (auto s : h->stage) cudaFree(s);
     delete h;
     return LBM_OK;
 }
-
-#define NEED(h) do { if (!(h)) return fail(LBM_ERR_INVALID, "%s: null handle", __func__); } while (0)
-#define LAUNCHED(h) do { CUDA_TRY(cudaGetLastError()); (h)->launches++; } while (0)
-
-static dim3 site_grid(const lbm_t *h, int tx) { return dim3((h->Lx + tx - 1) / tx, h->Lz, 1); }
 
 int lbm_init_rt(lbm_t *h, uint64_t seed, const lbm_rt_init *ic, void *stream)
 {
@@ -218,10 +450,13 @@ int lbm_init_rt(lbm_t *h, uint64_t seed, const lbm_rt_init *ic, void *stream)
     CUDA_TRY(cudaMemcpyAsync(h->d_hlo(), h_lo.data(), sizeof(double) * h->Lx, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(h->d_hhi(), h_hi.data(), sizeof(double) * h->Lx, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaStreamSynchronize(st));  // the host vectors go out of scope
-    lbm::RtArgs a{h->g, 1.0 / ic->T_d, 1.0 / ic->T_m, 1.0 / ic->T_u, ic->rho_m, ic->delta, ic->smooth_w};
-    lbm::init_rt_kernel<<<site_grid(h, lbm::AUX_TX), lbm::AUX_TX, 0, st>>>(h->buf[h->cur], h->layout(), a, h->d_hlo(), h->d_hhi());
+    lbm::RtArgs a{h->g, 1.0 / ic->T_d, 1.0 / ic->T_m, 1.0 / ic->T_u, ic->rho_m, ic->delta, ic->smooth_w,
+                  h->Lz_glob, h->z0 - h->glo};
+    // all stored rows: a slab's ghost rows start from the same closed form as its neighbours' own rows
+    lbm::init_rt_kernel<<<dim3((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->Lz), lbm::AUX_TX, 0, st>>>(
+        h->buf[h->cur], h->layout(), a, h->d_hlo(), h->d_hhi());
     LAUNCHED(h);
-    h->steps = 0;
+    h->steps = 0; h->layout_m = false; h->wrap_ok[h->cur] = false; h->slab_phase = 0;
     return LBM_OK;
 }
 
@@ -229,10 +464,10 @@ int lbm_init_equilibrium(lbm_t *h, const double *rho, const double *ux, const do
 {
     NEED(h);
     if (!rho || !ux || !uz || !T) return fail(LBM_ERR_INVALID, "lbm_init_equilibrium: null field");
-    lbm::init_equilibrium_kernel<<<site_grid(h, lbm::AUX_TX), lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
+    lbm::init_equilibrium_kernel<<<own_grid(h, lbm::AUX_TX), lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
         h->buf[h->cur], h->layout(), rho, ux, uz, T);
     LAUNCHED(h);
-    h->steps = 0;
+    h->steps = 0; h->layout_m = false; h->wrap_ok[h->cur] = false; h->slab_phase = 0;
     return LBM_OK;
 }
 
@@ -240,9 +475,11 @@ int lbm_set_populations(lbm_t *h, const double *f_dev, void *stream)
 {
     NEED(h);
     if (!f_dev) return fail(LBM_ERR_INVALID, "lbm_set_populations: null pointer");
-    dim3 grid((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->Lz, LBM_NPOP);
-    lbm::pack_kernel<<<grid, lbm::AUX_TX, 0, (cudaStream_t)stream>>>(h->buf[h->cur], h->layout(), f_dev);
+    dim3 grid((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->nz, LBM_NPOP);
+    h->layout_m = false;                 // the uploaded state is stored in the ordinary layout
+    lbm::pack_kernel<<<grid, lbm::AUX_TX, 0, (cudaStream_t)stream>>>(h->buf[h->cur], h->layout(), f_dev, 0);
     LAUNCHED(h);
+    h->wrap_ok[h->cur] = false; h->slab_phase = 0;
     return LBM_OK;
 }
 
@@ -250,22 +487,37 @@ int lbm_get_populations(lbm_t *h, double *f_dev, void *stream)
 {
     NEED(h);
     if (!f_dev) return fail(LBM_ERR_INVALID, "lbm_get_populations: null pointer");
-    dim3 grid((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->Lz, LBM_NPOP);
-    lbm::unpack_kernel<<<grid, lbm::AUX_TX, 0, (cudaStream_t)stream>>>(h->buf[h->cur], h->layout(), f_dev);
+    dim3 grid((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->nz, LBM_NPOP);
+    lbm::unpack_kernel<<<grid, lbm::AUX_TX, 0, (cudaStream_t)stream>>>(h->buf[h->cur], h->layout(), f_dev, 0);
     LAUNCHED(h);
     return LBM_OK;
 }
 
-// host variants stage through the OTHER lattice copy (free between steps), so no extra device memory
+// Host variants.  Two copies: the whole dense array is staged in the OTHER lattice copy (free between steps), so no
+// extra device memory.  One copy (in-place): one dense population plane at a time through a plane-sized buffer.
 int lbm_set_populations_host(lbm_t *h, const double *f_host, void *stream)
 {
     NEED(h);
     if (!f_host) return fail(LBM_ERR_INVALID, "lbm_set_populations_host: null pointer");
     cudaStream_t st = (cudaStream_t)stream;
-    double *tmp = h->buf[h->cur ^ 1];
-    CUDA_TRY(cudaMemcpyAsync(tmp, f_host, sizeof(double) * LBM_NPOP * h->Lx * h->Lz, cudaMemcpyHostToDevice, st));
-    int rc = lbm_set_populations(h, tmp, stream);
-    if (rc) return rc;
+    const size_t plane_elems = (size_t)h->Lx * h->nz;
+    if (!h->inplace) {
+        double *tmp = h->ubuf[h->cur ^ 1];
+        CUDA_TRY(cudaMemcpyAsync(tmp, f_host, sizeof(double) * LBM_NPOP * plane_elems, cudaMemcpyHostToDevice, st));
+        int rc = lbm_set_populations(h, tmp, stream);
+        if (rc) return rc;
+        h->wrap_ok[h->cur ^ 1] = false;
+    } else {
+        if (!h->plane_stage) CUDA_TRY(cudaMalloc(&h->plane_stage, sizeof(double) * plane_elems));
+        h->layout_m = false;
+        dim3 grid((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->nz, 1);
+        for (int l = 0; l < LBM_NPOP; ++l) {
+            CUDA_TRY(cudaMemcpyAsync(h->plane_stage, f_host + l * plane_elems, sizeof(double) * plane_elems, cudaMemcpyHostToDevice, st));
+            lbm::pack_kernel<<<grid, lbm::AUX_TX, 0, st>>>(h->buf[h->cur], h->layout(), h->plane_stage, l);
+            LAUNCHED(h);
+        }
+        h->wrap_ok[h->cur] = false;
+    }
     CUDA_TRY(cudaStreamSynchronize(st));
     return LBM_OK;
 }
@@ -275,10 +527,22 @@ int lbm_get_populations_host(lbm_t *h, double *f_host, void *stream)
     NEED(h);
     if (!f_host) return fail(LBM_ERR_INVALID, "lbm_get_populations_host: null pointer");
     cudaStream_t st = (cudaStream_t)stream;
-    double *tmp = h->buf[h->cur ^ 1];
-    int rc = lbm_get_populations(h, tmp, stream);
-    if (rc) return rc;
-    CUDA_TRY(cudaMemcpyAsync(f_host, tmp, sizeof(double) * LBM_NPOP * h->Lx * h->Lz, cudaMemcpyDeviceToHost, st));
+    const size_t plane_elems = (size_t)h->Lx * h->nz;
+    if (!h->inplace) {
+        double *tmp = h->ubuf[h->cur ^ 1];
+        int rc = lbm_get_populations(h, tmp, stream);
+        if (rc) return rc;
+        h->wrap_ok[h->cur ^ 1] = false;
+        CUDA_TRY(cudaMemcpyAsync(f_host, tmp, sizeof(double) * LBM_NPOP * plane_elems, cudaMemcpyDeviceToHost, st));
+    } else {
+        if (!h->plane_stage) CUDA_TRY(cudaMalloc(&h->plane_stage, sizeof(double) * plane_elems));
+        dim3 grid((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->nz, 1);
+        for (int l = 0; l < LBM_NPOP; ++l) {
+            lbm::unpack_kernel<<<grid, lbm::AUX_TX, 0, st>>>(h->buf[h->cur], h->layout(), h->plane_stage, l);
+            LAUNCHED(h);
+            CUDA_TRY(cudaMemcpyAsync(f_host + l * plane_elems, h->plane_stage, sizeof(double) * plane_elems, cudaMemcpyDeviceToHost, st));
+        }
+    }
     CUDA_TRY(cudaStreamSynchronize(st));
     return LBM_OK;
 }
@@ -287,70 +551,170 @@ int lbm_step(lbm_t *h, int n, void *stream)
 {
     NEED(h);
     if (n < 0) return fail(LBM_ERR_INVALID, "lbm_step: n must be >= 0 (got %d)", n);
+    if (h->slab) return fail(LBM_ERR_INVALID, "lbm_step: a z-slab is stepped with lbm_slab_step (its ghost rows must be exchanged every step)");
     cudaStream_t st = (cudaStream_t)stream;
-    lbm::StepArgs a;
-    a.Lx = h->Lx; a.Lz = h->Lz; a.pitch = h->pitch; a.plane = h->plane;
-    a.omega = 1.0 / h->tau;
-    a.gtau = h->g * h->tau;
-    a.dT = 0.5 * h->tau * (1.0 - h->tau) * h->g * h->g;
-    lbm::fill_offsets(a);
-    // Variants: 0 = automatic (two steps per launch where the lattice is large enough to fill the GPU with
-    // strips, else one step per launch), 1 = one step, 256x1 blocks, 2 = one step, 128x1 blocks,
+    lbm::StepArgs a = step_args(h);
+    // Variants: 0 = automatic (make_plan), 1 = one step per launch, 256x1 blocks, 2 = one step, 128x1 blocks,
     // 3 = two steps per launch forced.  An odd last step always runs the one-step kernel.
     using S2 = lbm::Step2sWide;
-    int ZC = h->zchunk;
-    const int strips = (h->Lx + S2::TX - 1) / S2::TX;
-    if (ZC == 0) {  // enough blocks for >= 6 waves over the SMs (the tail of the last wave is what costs on mid-size
-                    // lattices: 1024x2048 gains 8 % over 4 waves), chunks of 24..192 rows (warm-up is 6 rows per chunk)
-        const int want_chunks = (6 * h->sm_count + strips - 1) / strips;
-        ZC = (h->Lz + want_chunks - 1) / want_chunks;
-        ZC = (ZC + 5) / 6 * 6;   // whole passes for R = 2 or 3 rows
-        if (ZC < 24) ZC = 24;
-        if (ZC > 192) ZC = 192;
-    }
-    const long long blocks2 = (long long)strips * ((h->Lz + ZC - 1) / ZC);
-    const bool fused = h->variant == 3 ||
-                       (h->variant == 0 && h->tma_ok && blocks2 >= 2LL * h->sm_count && h->Lx >= 2 * S2::TX);
-    if (h->variant == 3 && !h->tma_ok)
-        return fail(LBM_ERR_CUDA, "lbm_step: the two-step kernel needs tensor maps (cuTensorMapEncodeTiled failed)");
+    const lbm_plan &plan = make_plan(h);
+    if (h->variant == 3 && !plan.fused)
+        return fail(LBM_ERR_CUDA, "lbm_step: the two-step kernel needs two lattice copies and tensor maps%s",
+                    h->tma_ok ? "" : " (cuTensorMapEncodeTiled failed)");
+    const int launches = plan.fused ? n / 2 + n % 2 : n;
+    // Under stream capture the handle's bookkeeping (which copy is current) advances at capture time, not at replay:
+    // a captured sequence must leave the current copy / layout where it was, i.e. hold an even number of launches.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+    if (cap != cudaStreamCaptureStatusNone && launches % 2)
+        return fail(LBM_ERR_INVALID, "lbm_step: %d steps are %d launches here; a captured sequence must hold an even "
+                    "number of launches (the ping-pong must return to the same copy)", n, launches);
     int s = 0;
-    if (fused && n >= 2) {
-        static bool attr_set = false;
-        if (!attr_set) {
-            CUDA_TRY(cudaFuncSetAttribute(lbm::step2s_kernel<S2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2::SMEM));
-            attr_set = true;
+    if (plan.fused && n >= 2) {
+        dim3 grid(plan.strips, plan.chunks);
+        a.w = plan.w;
+        // the consumers' spare lanes of the two seam strips keep the wrap columns of the destination current, if the
+        // seam columns [0, XW) and [Lx - XW, Lx) each lie within one strip and that strip has XW lanes to spare (2 XW
+        // if it is the only strip); else the columns are refreshed before every launch
+        {
+            const int last = h->Lx - (plan.strips - 1) * plan.w;      // columns of the last strip
+            a.wrap_store = h->Lx >= 2 * lbm::XW && last >= lbm::XW &&
+                           (plan.strips > 1 ? plan.w + lbm::XW <= S2::CW : last + 2 * lbm::XW <= S2::CW);
         }
-        dim3 grid(strips, (h->Lz + ZC - 1) / ZC);
         for (; s + 2 <= n; s += 2) {
+            int rc = refresh_wrap_columns(h, h->cur, st);
+            if (rc) return rc;
             a.src = h->buf[h->cur];
             a.dst = h->buf[h->cur ^ 1];
-            lbm::step2s_kernel<S2><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], ZC);
+            if (h->wall_kind == 1)
+                lbm::step2s_kernel<S2, true><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], plan.ZC);
+            else
+                lbm::step2s_kernel<S2, false><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], plan.ZC);
             LAUNCHED(h);
-            h->cur ^= 1;  // a5: swap prv / nxt, once per two steps
-            h->steps += 2;
+            h->wrap_ok[h->cur ^ 1] = a.wrap_store != 0;   // the consumers of the seam strips wrote the images
+            advance(h, 2);                               // a5: swap prv / nxt, once per two steps
         }
     }
     for (; s < n; ++s) {
-        a.src = h->buf[h->cur];
-        a.dst = h->buf[h->cur ^ 1];
-        // 128-thread blocks are a few per cent faster on the small (L2-resident, few-wave) lattices, 256 on the large
-        if (h->variant == 2 || (h->variant == 0 && (long long)h->Lx * h->Lz < (1LL << 20)))
-            lbm::step_kernel_site<128, 1><<<dim3((h->Lx + 127) / 128, h->Lz), dim3(128, 1), 0, st>>>(a);
-        else  // 256 threads = 2 blocks/SM at 128 registers: fastest one-step shape at 4096x8192
-            lbm::step_kernel_site<256, 1><<<dim3((h->Lx + 255) / 256, h->Lz), dim3(256, 1), 0, st>>>(a);
-        LAUNCHED(h);
-        h->cur ^= 1;  // a5: swap prv / nxt
-        h->steps++;
+        int rc = one_step_rows(h, a, 0, h->Lz, st);
+        if (rc) return rc;
+        h->wrap_ok[h->inplace ? h->cur : h->cur ^ 1] = false;
+        advance(h, 1);                                   // a5
     }
     return LBM_OK;
 }
 
+int lbm_get_plan(lbm_t *h, int *fused, int *strip_width, int *zchunk)
+{
+    NEED_HOST(h);
+    const lbm_plan &p = make_plan(h);
+    if (fused) *fused = p.fused ? 1 : 0;
+    if (strip_width) *strip_width = p.w;
+    if (zchunk) *zchunk = p.ZC;
+    return LBM_OK;
+}
+
+// ---- z-slabs (Fig. 3-4) -------------------------------------------------------
+int lbm_slab_info(const lbm_t *h, int *z0, int *nz, int *open_below, int *open_above, size_t *message_doubles)
+{
+    NEED_HOST(h);
+    if (!h->slab) return fail(LBM_ERR_INVALID, "lbm_slab_info: not a slab handle");
+    if (z0) *z0 = h->z0;
+    if (nz) *nz = h->nz;
+    if (open_below) *open_below = h->glo > 0;
+    if (open_above) *open_above = h->ghi > 0;
+    if (message_doubles) *message_doubles = (size_t)26 * h->Lx;
+    return LBM_OK;
+}
+
+int lbm_slab_pack(lbm_t *h, int side, double *msg_dev, void *stream)
+{
+    NEED(h);
+    if (!h->slab || (side != 0 && side != 1) || !msg_dev) return fail(LBM_ERR_INVALID, "lbm_slab_pack: slab handle, side 0/1 and a buffer are required");
+    if (side == 0 ? h->glo == 0 : h->ghi == 0) return fail(LBM_ERR_INVALID, "lbm_slab_pack: side %d of this slab is a wall", side);
+    lbm::slab_pack_kernel<<<dim3((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, 26), lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
+        h->buf[h->cur], h->layout(), slab_rows(h, side, true), msg_dev);
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
+int lbm_slab_unpack(lbm_t *h, int side, const double *msg_dev, void *stream)
+{
+    NEED(h);
+    if (!h->slab || (side != 0 && side != 1) || !msg_dev) return fail(LBM_ERR_INVALID, "lbm_slab_unpack: slab handle, side 0/1 and a buffer are required");
+    if (side == 0 ? h->glo == 0 : h->ghi == 0) return fail(LBM_ERR_INVALID, "lbm_slab_unpack: side %d of this slab is a wall", side);
+    lbm::slab_unpack_kernel<<<dim3((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, 26), lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
+        h->buf[h->cur], h->layout(), slab_rows(h, side, false), msg_dev);
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
+int lbm_slab_step(lbm_t *h, int part, void *stream)
+{
+    NEED(h);
+    if (!h->slab) return fail(LBM_ERR_INVALID, "lbm_slab_step: not a slab handle");
+    cudaStream_t st = (cudaStream_t)stream;
+    lbm::StepArgs a = step_args(h);
+    // own rows that read no ghost row: at least GHOST rows away from an open side
+    const int i0 = h->glo + (h->glo ? GHOST : 0), i1 = h->glo + h->nz - (h->ghi ? GHOST : 0);
+    if (part == LBM_SLAB_INTERIOR) {
+        if (h->slab_phase != 0) return fail(LBM_ERR_INVALID, "lbm_slab_step: interior rows of this step were already launched");
+        int rc = one_step_rows(h, a, i0, i1, st);
+        if (rc) return rc;
+        h->slab_phase = 1;
+        return LBM_OK;
+    }
+    if (part == LBM_SLAB_EDGES) {
+        if (h->slab_phase != 1) return fail(LBM_ERR_INVALID, "lbm_slab_step: launch the interior rows first");
+        int rc = one_step_rows(h, a, h->glo, i0, st);
+        if (!rc) rc = one_step_rows(h, a, i1, h->glo + h->nz, st);
+        if (rc) return rc;
+        h->slab_phase = 0;
+        h->wrap_ok[h->cur ^ 1] = false;
+        advance(h, 1);                                   // a5
+        return LBM_OK;
+    }
+    return fail(LBM_ERR_INVALID, "lbm_slab_step: part must be LBM_SLAB_INTERIOR or LBM_SLAB_EDGES (got %d)", part);
+}
+
+// ---- diagnostics (a6) ------------------------------------------------------------------------------------------------
 int lbm_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *stream)
 {
     NEED(h);
-    lbm::moments_kernel<<<site_grid(h, lbm::AUX_TX), lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
+    if (!rho && !ux && !uz && !T) return fail(LBM_ERR_INVALID, "lbm_moments: all four outputs are null");
+    lbm::moments_kernel<<<own_grid(h, lbm::AUX_TX), lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
         h->buf[h->cur], h->layout(), h->g, rho, ux, uz, T);
     LAUNCHED(h);
+    return LBM_OK;
+}
+
+// one pass over the lattice + one small block; results stay in the handle's scratch
+static int run_diagnostics(lbm_t *h, bool want_rms, double T_d, double T_m, double T_u, cudaStream_t st)
+{
+    if (want_rms) lbm::row_diagnostics_kernel<true><<<h->nz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, h->d_rows());
+    else lbm::row_diagnostics_kernel<false><<<h->nz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, h->d_rows());
+    LAUNCHED(h);
+    lbm::final_diagnostics_kernel<<<1, lbm::RED_T, 0, st>>>(h->d_rows(), h->nz, T_d, T_m, T_u, h->d_result());
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
+int lbm_diagnostics(lbm_t *h, double T_d, double T_m, double T_u, double *widths2, double *totals4, double *Tbar,
+                    double *Trms, double *Ekbar, double *Ekrms, void *stream)
+{
+    NEED(h);
+    if (widths2 && (T_m == T_u || T_d == T_m)) return fail(LBM_ERR_INVALID, "lbm_diagnostics: layer temperatures must differ");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = run_diagnostics(h, Trms || Ekrms, T_d, T_m, T_u, st);
+    if (rc) return rc;
+    double res[6];
+    CUDA_TRY(cudaMemcpyAsync(res, h->d_result(), sizeof res, cudaMemcpyDeviceToHost, st));
+    double *out[4] = {Tbar, Trms, Ekbar, Ekrms};
+    for (int j = 0; j < 4; ++j)
+        if (out[j]) CUDA_TRY(cudaMemcpyAsync(out[j], h->d_rows() + (long long)j * h->nz, sizeof(double) * h->nz, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (widths2) { widths2[0] = res[0]; widths2[1] = res[1]; }
+    if (totals4) for (int j = 0; j < 4; ++j) totals4[j] = res[2 + j];
     return LBM_OK;
 }
 
@@ -359,32 +723,25 @@ int lbm_mixing_widths(lbm_t *h, double T_d, double T_m, double T_u, double *L_u,
     NEED(h);
     if (!L_u || !L_d) return fail(LBM_ERR_INVALID, "lbm_mixing_widths: null output");
     if (T_m == T_u || T_d == T_m) return fail(LBM_ERR_INVALID, "lbm_mixing_widths: layer temperatures must differ");
-    cudaStream_t st = (cudaStream_t)stream;
-    lbm::row_tbar_kernel<<<h->Lz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, h->d_tbar());
-    LAUNCHED(h);
-    lbm::widths_kernel<<<1, lbm::RED_T, 0, st>>>(h->d_tbar(), h->Lz, T_d, T_m, T_u, h->d_result());
-    LAUNCHED(h);
-    double res[2];
-    CUDA_TRY(cudaMemcpyAsync(res, h->d_result(), sizeof res, cudaMemcpyDeviceToHost, st));
-    if (Tbar) CUDA_TRY(cudaMemcpyAsync(Tbar, h->d_tbar(), sizeof(double) * h->Lz, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    *L_u = res[0];
-    *L_d = res[1];
+    double w[2];
+    int rc = lbm_diagnostics(h, T_d, T_m, T_u, w, nullptr, Tbar, nullptr, nullptr, nullptr, stream);
+    if (rc) return rc;
+    *L_u = w[0];
+    *L_d = w[1];
     return LBM_OK;
 }
 
 int lbm_profiles(lbm_t *h, double *Tbar, double *Trms, double *Ekbar, double *Ekrms, void *stream)
 {
     NEED(h);
-    cudaStream_t st = (cudaStream_t)stream;
-    double *d = h->d_partial();  // [4][Lz], shared with the totals partials
-    lbm::row_profiles_kernel<<<h->Lz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, d);
-    LAUNCHED(h);
-    double *out[4] = {Tbar, Trms, Ekbar, Ekrms};
-    for (int j = 0; j < 4; ++j)
-        if (out[j]) CUDA_TRY(cudaMemcpyAsync(out[j], d + (long long)j * h->Lz, sizeof(double) * h->Lz, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    return LBM_OK;
+    return lbm_diagnostics(h, 0.0, 0.0, 0.0, nullptr, nullptr, Tbar, Trms, Ekbar, Ekrms, stream);
+}
+
+int lbm_totals(lbm_t *h, double *out4, void *stream)
+{
+    NEED(h);
+    if (!out4) return fail(LBM_ERR_INVALID, "lbm_totals: null output");
+    return lbm_diagnostics(h, 0.0, 0.0, 0.0, nullptr, out4, nullptr, nullptr, nullptr, nullptr, stream);
 }
 
 int lbm_growth_rate(int n, const double *t, const double *L, double g, double At, double *alpha)
@@ -400,6 +757,15 @@ int lbm_growth_rate(int n, const double *t, const double *L, double g, double At
         }
         alpha[j] = L[j] > 0.0 ? (slope * slope) / (4.0 * g * At * L[j]) : 0.0;
     }
+    return LBM_OK;
+}
+
+int lbm_rt_scales(double Lx, double g, double T_d, double T_u, double *At, double *tau_rt)
+{
+    if (!(Lx > 0.0) || !(g > 0.0) || !(T_d > T_u) || !(T_u > 0.0)) return fail(LBM_ERR_INVALID, "lbm_rt_scales: need Lx, g > 0 and T_d > T_u > 0");
+    const double a = (T_d - T_u) / (T_d + T_u);
+    if (At) *At = a;
+    if (tau_rt) *tau_rt = std::sqrt(Lx / (g * a));
     return LBM_OK;
 }
 
@@ -433,25 +799,12 @@ int lbm_fp64_peak(double *tflops, int iters, void *stream)
     return LBM_OK;
 }
 
-int lbm_totals(lbm_t *h, double *out4, void *stream)
-{
-    NEED(h);
-    if (!out4) return fail(LBM_ERR_INVALID, "lbm_totals: null output");
-    cudaStream_t st = (cudaStream_t)stream;
-    lbm::row_totals_kernel<<<h->Lz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->d_partial());
-    LAUNCHED(h);
-    lbm::final_totals_kernel<<<1, lbm::RED_T, 0, st>>>(h->d_partial(), h->Lz, h->d_result() + 2);
-    LAUNCHED(h);
-    CUDA_TRY(cudaMemcpyAsync(out4, h->d_result() + 2, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    return LBM_OK;
-}
-
 int lbm_run_host(lbm_t *h, const double *rho_in, const double *ux_in, const double *uz_in, const double *T_in, int n,
                  double *rho_out, double *ux_out, double *uz_out, double *T_out, void *stream)
 {
     NEED(h);
     if (!rho_in || !ux_in || !uz_in || !T_in) return fail(LBM_ERR_INVALID, "lbm_run_host: null input field");
+    if (h->slab) return fail(LBM_ERR_INVALID, "lbm_run_host: not available for z-slabs");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = sizeof(double) * (size_t)h->Lx * h->Lz;
     for (auto &s : h->stage)
@@ -463,9 +816,11 @@ int lbm_run_host(lbm_t *h, const double *rho_in, const double *ux_in, const doub
     rc = lbm_step(h, n, stream);
     if (rc) return rc;
     double *out[4] = {rho_out, ux_out, uz_out, T_out};
-    rc = lbm_moments(h, out[0] ? h->stage[0] : nullptr, out[1] ? h->stage[1] : nullptr, out[2] ? h->stage[2] : nullptr,
-                     out[3] ? h->stage[3] : nullptr, stream);
-    if (rc) return rc;
+    if (out[0] || out[1] || out[2] || out[3]) {
+        rc = lbm_moments(h, out[0] ? h->stage[0] : nullptr, out[1] ? h->stage[1] : nullptr, out[2] ? h->stage[2] : nullptr,
+                         out[3] ? h->stage[3] : nullptr, stream);
+        if (rc) return rc;
+    }
     for (int j = 0; j < 4; ++j)
         if (out[j]) CUDA_TRY(cudaMemcpyAsync(out[j], h->stage[j], bytes, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -474,14 +829,14 @@ int lbm_run_host(lbm_t *h, const double *rho_in, const double *ux_in, const doub
 
 int lbm_steps_done(const lbm_t *h, long long *steps)
 {
-    NEED(h);
+    NEED_HOST(h);
     if (steps) *steps = h->steps;
     return LBM_OK;
 }
 
 int lbm_layout(const lbm_t *h, int *pitch, long long *plane_stride)
 {
-    NEED(h);
+    NEED_HOST(h);
     if (pitch) *pitch = h->pitch;
     if (plane_stride) *plane_stride = h->plane;
     return LBM_OK;
@@ -489,26 +844,28 @@ int lbm_layout(const lbm_t *h, int *pitch, long long *plane_stride)
 
 int lbm_kernel_launches(const lbm_t *h, long long *launches)
 {
-    NEED(h);
+    NEED_HOST(h);
     if (launches) *launches = h->launches;
     return LBM_OK;
 }
 
 int lbm_set_zchunk(lbm_t *h, int rows)
 {
-    NEED(h);
+    NEED_HOST(h);
     // chunks above the first must start at row >= 3: only the chunk at z0 = 0 builds the bottom wall's ghost rows
     if (rows < 0 || rows == 1 || rows == 2)
         return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be 0 (automatic) or >= 3 (got %d)", rows);
     h->zchunk = rows;
+    h->plan.valid = false;
     return LBM_OK;
 }
 
 int lbm_set_variant(lbm_t *h, int variant)
 {
-    NEED(h);
+    NEED_HOST(h);
     if (variant < 0 || variant > 3) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
     h->variant = variant;
+    h->plan.valid = false;
     return LBM_OK;
 }
 

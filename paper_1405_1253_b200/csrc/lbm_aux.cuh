@@ -1,4 +1,5 @@
-// lbm_aux.cuh -- initial states, layout conversion and the moments / diagnostics kernels (row a6).
+// lbm_aux.cuh -- initial states, layout conversion, wrap-column refresh, z-slab messages and the moments /
+// diagnostics kernels (row a6).
 #pragma once
 #include <cstdint>
 
@@ -7,21 +8,24 @@
 
 namespace lbm {
 
+// The stored lattice as the aux kernels see it.  `buf` points at site (0, 0) of population 0 (the wrap columns of
+// DESIGN.md section 5 lie at negative column offsets).  Dense user arrays cover the OWNED rows only: rows
+// [k0, k0 + nz) of the stored lattice (a whole lattice owns all its rows; a z-slab also stores ghost rows).
 struct Layout {
     int Lx, Lz, pitch;
     long long plane;
+    int k0, nz;
+    bool layout_m;      // in-place path after an odd number of steps (lbm_step.cuh)
 };
 
 constexpr int AUX_TX = 128;  // threads per block along x for the per-site aux kernels
 constexpr int RED_T = 256;   // threads per block of the row reductions
 
+// the 37 populations of stored site (i, k), whatever the layout
 __device__ __forceinline__ void load_site(const double *src, const Layout &g, int i, int k, double (&f)[NPOP])
 {
-    const double *p = src + (long long)k * g.pitch + i;
-    d2q37::static_for<0, NPOP>([&](auto L) {
-        constexpr int l = decltype(L)::value;
-        f[l] = __ldg(p + (long long)l * g.plane);
-    });
+    each_stored_site(src, g.Lx, g.Lz, g.pitch, g.plane, g.layout_m, i, k,
+                     [&](auto L, const double *p) { f[decltype(L)::value] = __ldg(p); });
 }
 
 __device__ __forceinline__ void store_site(double *dst, const Layout &g, int i, int k, const double (&f)[NPOP])
@@ -33,23 +37,25 @@ __device__ __forceinline__ void store_site(double *dst, const Layout &g, int i, 
     });
 }
 
-// populations = f_eq(rho, u, T) of given kinetic fields (dense [Lz][Lx])
+// populations = f_eq(rho, u, T) of given kinetic fields (dense [nz][Lx]); grid.y = nz
 __global__ void __launch_bounds__(AUX_TX)
 init_equilibrium_kernel(double *dst, Layout g, const double *__restrict__ rho, const double *__restrict__ ux,
                         const double *__restrict__ uz, const double *__restrict__ T)
 {
-    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y;
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y;
     if (i >= g.Lx) return;
-    const long long s = (long long)k * g.Lx + i;
+    const long long s = (long long)j * g.Lx + i;
     double f[NPOP];
     d2q37::equilibrium_blend<false>(f, f, 0.0, rho[s], ux[s], uz[s], T[s]);
-    store_site(dst, g, i, k, f);
+    store_site(dst, g, i, g.k0 + j, f);
 }
 
 // Hydrostatic three-layer state, eq. 1-2 with tanh-smoothed jumps;
-// DESIGN.md reading 11.  z_k = k - (Lz-1)/2 in sites, one site = r length units, beta = 1/T0.
+// DESIGN.md reading 11.  z_k = k - (Lz-1)/2 in sites of the GLOBAL lattice, one site = r length units, beta = 1/T0.
 struct RtArgs {
     double g, beta_d, beta_m, beta_u, rho_m, delta, w;
+    int Lz_glob;        // height of the whole lattice
+    int zshift;         // global row of stored row 0 (0 for a whole lattice; a slab stores ghost rows below its own)
 };
 
 __device__ __forceinline__ double rt_lncosh(double s)
@@ -68,12 +74,13 @@ __device__ __forceinline__ double rt_step_integral(double z, double a, double w)
     return fmax(z - a, 0.0) - fmax(-a, 0.0);
 }
 
+// grid.y = all stored rows (a slab's ghost rows are initialised from the same closed form)
 __global__ void __launch_bounds__(AUX_TX)
 init_rt_kernel(double *dst, Layout g, RtArgs p, const double *__restrict__ h_lo, const double *__restrict__ h_hi)
 {
     const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y;
     if (i >= g.Lx) return;
-    const double z = (double)k - 0.5 * (double)(g.Lz - 1);
+    const double z = (double)(k + p.zshift) - 0.5 * (double)(p.Lz_glob - 1);
     const double a_lo = -0.5 * p.delta + h_lo[i], a_hi = 0.5 * p.delta + h_hi[i];
     const double dlo = p.beta_m - p.beta_d, dhi = p.beta_u - p.beta_m;
     const double beta = p.beta_d + dlo * rt_step(z, a_lo, p.w) + dhi * rt_step(z, a_hi, p.w);
@@ -88,31 +95,71 @@ init_rt_kernel(double *dst, Layout g, RtArgs p, const double *__restrict__ h_lo,
     store_site(dst, g, i, k, f);
 }
 
-// canonical dense [37][Lz][Lx]  <->  padded layout; grid = (ceil(Lx/AUX_TX), Lz, 37)
-__global__ void __launch_bounds__(AUX_TX) pack_kernel(double *dst, Layout g, const double *__restrict__ dense)
+// canonical dense [nl][nz][Lx] (populations l0 .. l0+nl-1)  <->  the stored lattice; grid = (ceil(Lx/AUX_TX), nz, nl).
+// pack always writes the ordinary layout; unpack reads either layout.
+__global__ void __launch_bounds__(AUX_TX) pack_kernel(double *dst, Layout g, const double *__restrict__ dense, int l0)
 {
-    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y, l = blockIdx.z;
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y, l = l0 + blockIdx.z;
     if (i >= g.Lx) return;
-    dst[(long long)l * g.plane + (long long)k * g.pitch + i] = dense[((long long)l * g.Lz + k) * g.Lx + i];
+    dst[(long long)l * g.plane + (long long)(g.k0 + j) * g.pitch + i] = dense[((long long)blockIdx.z * g.nz + j) * g.Lx + i];
 }
-__global__ void __launch_bounds__(AUX_TX) unpack_kernel(const double *__restrict__ src, Layout g, double *dense)
+__global__ void __launch_bounds__(AUX_TX) unpack_kernel(const double *__restrict__ src, Layout g, double *dense, int l0)
 {
-    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y, l = blockIdx.z;
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y, l = l0 + blockIdx.z;
     if (i >= g.Lx) return;
-    dense[((long long)l * g.Lz + k) * g.Lx + i] = src[(long long)l * g.plane + (long long)k * g.pitch + i];
+    const double *p = nullptr;
+    each_stored_site(src, g.Lx, g.Lz, g.pitch, g.plane, g.layout_m, i, g.k0 + j, [&](auto L, const double *q) {
+        if (decltype(L)::value == l) p = q;
+    });
+    dense[((long long)blockIdx.z * g.nz + j) * g.Lx + i] = *p;
+}
+
+// a1 for the two-step kernel's TMA loads: the XW wrap columns on either side of a row hold the periodic images
+// (column j < 0 holds column j mod Lx, column Lx + j holds column j mod Lx).  The two-step kernel's consumers keep
+// them current themselves; this kernel refreshes them after anything else has written the lattice.
+// grid = Lz, block = NPOP x 2 XW threads (one row of all populations per block).
+template <int XW>
+__global__ void __launch_bounds__(2 * XW * NPOP) wrap_columns_kernel(double *buf, Layout g)
+{
+    double *row = buf + (long long)(threadIdx.x / (2 * XW)) * g.plane + (long long)blockIdx.x * g.pitch;
+    const int t = threadIdx.x % (2 * XW);
+    const int j = t < XW ? t - XW : g.Lx + t - XW;           // halo column
+    int s = j % g.Lx;
+    if (s < 0) s += g.Lx;
+    row[j] = row[s];
+}
+
+// z-slab messages (26 population-rows per direction).  The neighbour on `side` reads from its ghost
+// row at distance d = 1, 2, 3 only the populations that move towards it by at least d rows: 15 + 8 + 3 of them.
+// msg = [26][Lx]; entry j is population sel.l[j] of stored row sel.row[j].  grid = (ceil(Lx/AUX_TX), 26).
+struct SlabRows {
+    int row[26];
+    int l[26];
+};
+__global__ void __launch_bounds__(AUX_TX) slab_pack_kernel(const double *__restrict__ src, Layout g, SlabRows sel, double *msg)
+{
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y;
+    if (i >= g.Lx) return;
+    msg[(long long)j * g.Lx + i] = src[(long long)sel.l[j] * g.plane + (long long)sel.row[j] * g.pitch + i];
+}
+__global__ void __launch_bounds__(AUX_TX) slab_unpack_kernel(double *dst, Layout g, SlabRows sel, const double *__restrict__ msg)
+{
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y;
+    if (i >= g.Lx) return;
+    dst[(long long)sel.l[j] * g.plane + (long long)sel.row[j] * g.pitch + i] = msg[(long long)j * g.Lx + i];
 }
 
 // Hydrodynamic fields of the stored (post-collision) state: rho, u^(H) = u - g_vec dt/2 = (u_x, u_z + g/2),
-// T^(H) = T + g^2/8 (PAPER.md:94 applied after the collision's u -> u + g_vec dt; reading 8).
+// T^(H) = T + g^2/8 (PAPER.md:94 applied after the collision's u -> u + g_vec dt; reading 8).  grid.y = nz
 __global__ void __launch_bounds__(AUX_TX)
 moments_kernel(const double *__restrict__ src, Layout g, double grav, double *rho, double *ux, double *uz, double *T)
 {
-    const int i = blockIdx.x * AUX_TX + threadIdx.x, k = blockIdx.y;
+    const int i = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y;
     if (i >= g.Lx) return;
     double f[NPOP];
-    load_site(src, g, i, k, f);
+    load_site(src, g, i, g.k0 + j, f);
     const d2q37::Kinetic m = d2q37::kinetic_moments(f);
-    const long long s = (long long)k * g.Lx + i;
+    const long long s = (long long)j * g.Lx + i;
     if (rho) rho[s] = m.rho;
     if (ux) ux[s] = m.ux;
     if (uz) uz[s] = m.uz + 0.5 * grav;
@@ -133,60 +180,57 @@ __device__ __forceinline__ double block_sum(double v, double *smem /* RED_T/32 d
     return t;
 }
 
-// Tbar[k] = (1/Lx) sum_i T^(H)(i,k); one block per row
-__global__ void __launch_bounds__(RED_T) row_tbar_kernel(const double *__restrict__ src, Layout g, double grav, double *Tbar)
-{
-    __shared__ double sm[RED_T / 32];
-    const int k = blockIdx.x;
-    double acc = 0.0;
-    for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
-        double f[NPOP];
-        load_site(src, g, i, k, f);
-        acc += d2q37::kinetic_moments(f).T + 0.125 * grav * grav;
-    }
-    const double t = block_sum(acc, sm);
-    if (threadIdx.x == 0) Tbar[k] = t / (double)g.Lx;
-}
-
-// Row profiles of section IV (Fig. 8, Fig. 9): x-mean and x-rms of
-// T^(H) and of E_k = rho |u^(H)|^2 / 2 (reading 17).  One block per row, two passes (means, then
-// squared deviations; the second pass re-reads the row from L2), deterministic.  out = [4][Lz]:
-// Tbar | Trms | Ekbar | Ekrms.
-__global__ void __launch_bounds__(RED_T) row_profiles_kernel(const double *__restrict__ src, Layout g, double grav, double *out)
+// One pass over the lattice for every per-row diagnostic (one block per owned row, deterministic):
+//   out[0][j] = Tbar(j)  = <T^(H)>_x
+//   out[1][j] = Trms(j)  = sqrt(<(T - <T>_x)^2>_x)         (Fig. 8)
+//   out[2][j] = Ekbar(j) = <E_k>_x, E_k = rho |u^(H)|^2/2  (Fig. 9; reading 17)
+//   out[3][j] = Ekrms(j)
+//   out[4..7][j] = row sums of the raw integer-velocity moments sum f, sum e_x f, sum e_z f, sum |e|^2 f
+// WANT_RMS = false skips the second pass over the row (the squared deviations; it re-reads the row from L2).
+template <bool WANT_RMS>
+__global__ void __launch_bounds__(RED_T) row_diagnostics_kernel(const double *__restrict__ src, Layout g, double grav, double *out)
 {
     __shared__ double sm[RED_T / 32];
     __shared__ double mean[2];
-    const int k = blockIdx.x;
-    double aT = 0.0, aE = 0.0;
+    const int j = blockIdx.x, k = g.k0 + j;
+    double aT = 0.0, aE = 0.0, a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
         double f[NPOP];
         load_site(src, g, i, k, f);
-        const d2q37::Kinetic m = d2q37::kinetic_moments(f);
+        const d2q37::RawMoments r = d2q37::raw_moments(f);
+        const d2q37::Kinetic m = d2q37::kinetic_from_raw(r);
         const double uz = m.uz + 0.5 * grav;
         aT += m.T + 0.125 * grav * grav;
         aE += 0.5 * m.rho * (m.ux * m.ux + uz * uz);
+        a0 += r.m0; a1 += r.jx; a2 += r.jz; a3 += r.m2;
     }
     const double sT = block_sum(aT, sm), sE = block_sum(aE, sm);
-    if (threadIdx.x == 0) { mean[0] = sT / (double)g.Lx; mean[1] = sE / (double)g.Lx; }
-    __syncthreads();
-    const double mT = mean[0], mE = mean[1];
-    double vT = 0.0, vE = 0.0;
-    for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
-        double f[NPOP];
-        load_site(src, g, i, k, f);
-        const d2q37::Kinetic m = d2q37::kinetic_moments(f);
-        const double uz = m.uz + 0.5 * grav;
-        const double dT = m.T + 0.125 * grav * grav - mT;
-        const double dE = 0.5 * m.rho * (m.ux * m.ux + uz * uz) - mE;
-        vT += dT * dT;
-        vE += dE * dE;
-    }
-    const double qT = block_sum(vT, sm), qE = block_sum(vE, sm);
+    const double s0 = block_sum(a0, sm), s1 = block_sum(a1, sm), s2 = block_sum(a2, sm), s3 = block_sum(a3, sm);
     if (threadIdx.x == 0) {
-        out[k] = mT;
-        out[g.Lz + k] = sqrt(qT / (double)g.Lx);
-        out[2 * g.Lz + k] = mE;
-        out[3 * g.Lz + k] = sqrt(qE / (double)g.Lx);
+        mean[0] = sT / (double)g.Lx; mean[1] = sE / (double)g.Lx;
+        out[j] = mean[0];
+        out[2 * g.nz + j] = mean[1];
+        out[4 * g.nz + j] = s0; out[5 * g.nz + j] = s1; out[6 * g.nz + j] = s2; out[7 * g.nz + j] = s3;
+    }
+    if constexpr (WANT_RMS) {
+        __syncthreads();
+        const double mT = mean[0], mE = mean[1];
+        double vT = 0.0, vE = 0.0;
+        for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
+            double f[NPOP];
+            load_site(src, g, i, k, f);
+            const d2q37::Kinetic m = d2q37::kinetic_moments(f);
+            const double uz = m.uz + 0.5 * grav;
+            const double dT = m.T + 0.125 * grav * grav - mT;
+            const double dE = 0.5 * m.rho * (m.ux * m.ux + uz * uz) - mE;
+            vT += dT * dT;
+            vE += dE * dE;
+        }
+        const double qT = block_sum(vT, sm), qE = block_sum(vE, sm);
+        if (threadIdx.x == 0) {
+            out[g.nz + j] = sqrt(qT / (double)g.Lx);
+            out[3 * g.nz + j] = sqrt(qE / (double)g.Lx);
+        }
     }
 }
 
@@ -197,50 +241,28 @@ __device__ __forceinline__ double tent(double b)
     return b < 0.5 ? 2.0 * b : 2.0 * (1.0 - b);
 }
 
-// eq. 12: out[0] = L_u, out[1] = L_d, in sites; single block
+// Second stage, single block over the nz owned rows of the per-row array `rows` (row_diagnostics_kernel):
+//   res[0] = L_u, res[1] = L_d of eq. 12 from Tbar, in sites (skipped if T_m == T_u or T_d == T_m)
+//   res[2..5] = sum f, sum c_x f, sum c_z f, sum |c|^2 f, c = r e
 __global__ void __launch_bounds__(RED_T)
-widths_kernel(const double *__restrict__ Tbar, int Lz, double T_d, double T_m, double T_u, double *out)
+final_diagnostics_kernel(const double *__restrict__ rows, int nz, double T_d, double T_m, double T_u, double *res)
 {
     __shared__ double sm[RED_T / 32];
-    double lu = 0.0, ld = 0.0;
-    for (int k = threadIdx.x; k < Lz; k += RED_T) {
-        const double tb = Tbar[k];
-        lu += tent((tb - T_u) / (T_m - T_u));
-        ld += tent((tb - T_m) / (T_d - T_m));
+    const bool widths = T_m != T_u && T_d != T_m;
+    double lu = 0.0, ld = 0.0, a[4] = {0, 0, 0, 0};
+    for (int k = threadIdx.x; k < nz; k += RED_T) {
+        if (widths) {
+            const double tb = rows[k];
+            lu += tent((tb - T_u) / (T_m - T_u));
+            ld += tent((tb - T_m) / (T_d - T_m));
+        }
+        for (int j = 0; j < 4; ++j) a[j] += rows[(long long)(4 + j) * nz + k];
     }
-    const double a = block_sum(lu, sm);
-    const double b = block_sum(ld, sm);
-    if (threadIdx.x == 0) { out[0] = a; out[1] = b; }
-}
-
-// lattice totals, stage 1: per-row sums of the raw integer-velocity moments; partial[k][4]
-__global__ void __launch_bounds__(RED_T) row_totals_kernel(const double *__restrict__ src, Layout g, double *partial)
-{
-    __shared__ double sm[RED_T / 32];
-    const int k = blockIdx.x;
-    double a0 = 0, a1 = 0, a2 = 0, a3 = 0;
-    for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
-        double f[NPOP];
-        load_site(src, g, i, k, f);
-        const d2q37::RawMoments m = d2q37::raw_moments(f);
-        a0 += m.m0; a1 += m.jx; a2 += m.jz; a3 += m.m2;
-    }
-    const double s0 = block_sum(a0, sm), s1 = block_sum(a1, sm), s2 = block_sum(a2, sm), s3 = block_sum(a3, sm);
-    if (threadIdx.x == 0) {
-        partial[4 * k + 0] = s0; partial[4 * k + 1] = s1; partial[4 * k + 2] = s2; partial[4 * k + 3] = s3;
-    }
-}
-
-// stage 2: out = (sum f, sum c_x f, sum c_z f, sum |c|^2 f), c = r e; single block
-__global__ void __launch_bounds__(RED_T) final_totals_kernel(const double *__restrict__ partial, int Lz, double *out)
-{
-    __shared__ double sm[RED_T / 32];
-    double a[4] = {0, 0, 0, 0};
-    for (int k = threadIdx.x; k < Lz; k += RED_T)
-        for (int j = 0; j < 4; ++j) a[j] += partial[4 * k + j];
+    const double su = block_sum(lu, sm), sd = block_sum(ld, sm);
     const double s0 = block_sum(a[0], sm), s1 = block_sum(a[1], sm), s2 = block_sum(a[2], sm), s3 = block_sum(a[3], sm);
     if (threadIdx.x == 0) {
-        out[0] = s0; out[1] = D2Q37_R * s1; out[2] = D2Q37_R * s2; out[3] = D2Q37_R2 * s3;
+        res[0] = su; res[1] = sd;
+        res[2] = s0; res[3] = D2Q37_R * s1; res[4] = D2Q37_R * s2; res[5] = D2Q37_R2 * s3;
     }
 }
 

@@ -18,6 +18,9 @@ namespace lbm {
 
 using d2q37::NPOP;
 
+constexpr int XH = 16;   // spare columns stored on either side of every row (128 bytes: x = 0 stays on a 128-byte line)
+constexpr int XW = 8;    // ... of which the nearest XW hold the periodic images (the two-step kernel's boxes reach 8 out)
+
 struct StepArgs {
     const double *src;
     double *dst;
@@ -27,6 +30,12 @@ struct StepArgs {
     double omega;       // dt / tau
     double gtau;        // g tau
     double dT;          // tau (1 - tau) g^2 / 2
+    // isothermal no-slip walls (wall_kind 1, reading 19): flags per wall (0 for wall_kind 0 and for the
+    // open side of a z-slab), the imposed kinetic state u_w = (0, uwz), T_w per wall
+    int iso_lo, iso_hi;
+    double uwz, Tw_lo, Tw_hi;
+    int wrap_store;     // two-step kernel: the consumers of the seam strips maintain the wrap columns (Lx >= 2 XW)
+    int w;              // two-step kernel: columns per strip
     // byte offset of population l's pull source relative to the site's own address in plane 0, for sites that
     // need neither wrap nor wall remap: 8 (l plane - e_lz pitch - e_lx).  Host-computed (fill_offsets) so that
     // the kernel adds one opaque uniform constant per load instead of re-deriving it.
@@ -79,7 +88,7 @@ __device__ __forceinline__ void each_source_site(const StepArgs &a, int i, int k
         constexpr int ex = d2q37::pop_ex(l), ez = d2q37::pop_ez(l);
         int ls = l;
         if (WALL) ls = flip[ez + 3] ? (NPOP - 1 - l) : l;
-        fn(L, a.src + (long long)ls * a.plane + rowoff[ez + 3] + col[ex + 3]);
+        fn(L, a.src + (long long)ls * a.plane + rowoff[ez + 3] + col[ex + 3], WALL && flip[ez + 3]);
     });
 }
 
@@ -92,7 +101,7 @@ __device__ __forceinline__ void each_source_interior(const StepArgs &a, int i, i
     const char *p = reinterpret_cast<const char *>(a.src + (long long)k * a.pitch + i);
     d2q37::static_for<0, NPOP>([&](auto L) {
         constexpr int l = decltype(L)::value;
-        fn(L, reinterpret_cast<const double *>(p + a.gbyte[l]));
+        fn(L, reinterpret_cast<const double *>(p + a.gbyte[l]), false);
     });
 }
 
@@ -109,7 +118,17 @@ __device__ __forceinline__ void each_source_any(const StepArgs &a, int i, int k,
 // Gather the 37 post-propagate populations of site (i, k) into registers.
 __device__ __forceinline__ void gather_any(const StepArgs &a, int i, int k, double (&f)[NPOP])
 {
-    each_source_any(a, i, k, [&](auto L, const double *p) { f[decltype(L)::value] = ld_stream(p); });
+    each_source_any(a, i, k, [&](auto L, const double *p, bool) { f[decltype(L)::value] = ld_stream(p); });
+}
+
+// wall_kind 1: rows 0..2 / Lz-3..Lz-1 next to an isothermal wall get the wall state imposed after the gather (a3)
+template <bool ISO>
+__device__ __forceinline__ void wall_rows_adjust(const StepArgs &a, int k, double (&f)[NPOP])
+{
+    if constexpr (ISO) {
+        if (a.iso_lo && k < 3) d2q37::wall_adjust(f, a.uwz, a.Tw_lo);
+        else if (a.iso_hi && k >= a.Lz - 3) d2q37::wall_adjust(f, a.uwz, a.Tw_hi);
+    }
 }
 
 __device__ __forceinline__ void scatter_site(const StepArgs &a, int i, int k, const double (&f)[NPOP])
@@ -121,18 +140,105 @@ __device__ __forceinline__ void scatter_site(const StepArgs &a, int i, int k, co
     });
 }
 
-// One thread per site; a block covers TX consecutive columns of TZ consecutive rows,
-// grid = (ceil(Lx/TX), ceil(Lz/TZ)).  The wall test is per row, hence warp-uniform (TX is a multiple of 32).
-template <int TX, int TZ>
-__global__ void __launch_bounds__(TX *TZ, 512 / (TX * TZ)) step_kernel_site(const StepArgs a)
+// One thread per site; a block covers TX consecutive columns of TZ consecutive rows of the row range [k0, k1),
+// grid = (ceil(Lx/TX), ceil((k1-k0)/TZ)).  The wall test is per row, hence warp-uniform (TX is a multiple of 32).
+// ISO = true: the instance for wall_kind 1 (the adjustment sits in a block-uniform branch taken by six rows).
+template <int TX, int TZ, bool ISO>
+__global__ void __launch_bounds__(TX *TZ, 512 / (TX * TZ)) step_kernel_site(const StepArgs a, const int k0, const int k1)
 {
     const int i = blockIdx.x * TX + threadIdx.x;
-    const int k = blockIdx.y * TZ + threadIdx.y;
-    if (i >= a.Lx || k >= a.Lz) return;
+    const int k = k0 + blockIdx.y * TZ + threadIdx.y;
+    if (i >= a.Lx || k >= k1) return;
     double f[NPOP];
     gather_any(a, i, k, f);
+    wall_rows_adjust<ISO>(a, k, f);
     d2q37::collide_site(f, a.omega, a.gtau, a.dT);
     scatter_site(a, i, k, f);
+}
+
+// ---- in-place streaming: ONE lattice copy ("we keep in memory two copies of the lattice ... This choice
+// requires more memory").  Every site reads 37 slots and writes its 37 results back into the SAME slots, so no slot
+// is touched by two sites in a step and no second copy is needed.  Two alternating kernels:
+//   layout N (after an even number of steps):  A[l][x] = F_l(x), the stored post-collision state;
+//   EVEN step (N -> M): site x gathers f*_l(x) from the slots s(x,l) the ordinary pull reads (neighbour sites, wrap,
+//       wall remap), collides, and writes F'_{36-l}(x) into s(x,l) -- for a wall-reflected gather (slot in the mirror
+//       row, population 36-l) it writes F'_{(e_lx, -e_lz)}(x) instead, which is what makes the next step local;
+//   layout M:  A[l][y] = F'_{36-l}(y + e_l)  (and the x-flipped variant for the reflected slots);
+//   ODD step (M -> N): everything site x needs is at site x: f*_l(x) = A[36-l][x], or A[(e_lx, -e_lz)][x] where
+//       the pull source row k - e_lz lies beyond a wall; collide; write F''_l(x) to A[l][x].
+// Same gather values, same collision arithmetic: bit-identical to the two-copy kernels.
+template <int TX, bool ISO>
+__global__ void __launch_bounds__(TX, 512 / TX) step_inplace_even_kernel(const StepArgs a, const int k0, const int k1)
+{
+    const int i = blockIdx.x * TX + threadIdx.x;
+    const int k = k0 + blockIdx.y;
+    if (i >= a.Lx || k >= k1) return;
+    double f[NPOP];
+    gather_any(a, i, k, f);
+    wall_rows_adjust<ISO>(a, k, f);
+    d2q37::collide_site(f, a.omega, a.gtau, a.dT);
+    each_source_any(a, i, k, [&](auto L, const double *p, bool reflected) {
+        constexpr int l = decltype(L)::value;
+        constexpr int lx = d2q37::pop_index(d2q37::pop_ex(l), -d2q37::pop_ez(l));
+        st_stream(const_cast<double *>(p), reflected ? f[lx] : f[NPOP - 1 - l]);
+    });
+}
+
+template <int TX, bool ISO>
+__global__ void __launch_bounds__(TX, 512 / TX) step_inplace_odd_kernel(const StepArgs a, const int k0, const int k1)
+{
+    const int i = blockIdx.x * TX + threadIdx.x;
+    const int k = k0 + blockIdx.y;
+    if (i >= a.Lx || k >= k1) return;
+    double *p = a.dst + (long long)k * a.pitch + i;           // src == dst: the one copy
+    double f[NPOP];
+    const bool wall_row = k < 3 || k >= a.Lz - 3;             // block-uniform
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        constexpr int ez = d2q37::pop_ez(l);
+        constexpr int lx = d2q37::pop_index(d2q37::pop_ex(l), -ez);
+        int ls = NPOP - 1 - l;
+        if (wall_row && (k - ez < 0 || k - ez >= a.Lz)) ls = lx;
+        f[l] = ld_stream(p + (long long)ls * a.plane);
+    });
+    wall_rows_adjust<ISO>(a, k, f);
+    d2q37::collide_site(f, a.omega, a.gtau, a.dT);
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int l = decltype(L)::value;
+        st_stream(p + (long long)l * a.plane, f[l]);
+    });
+}
+
+// Population m of site (i, k) of the STORED state, for either layout of the in-place path (layout_m = false: the
+// ordinary layout, also that of the two-copy path).  Used by the diagnostics and by lbm_get_populations.
+template <class Fn>
+__device__ __forceinline__ void each_stored_site(const double *buf, int Lx, int Lz, int pitch, long long plane,
+                                                 bool layout_m, int i, int k, Fn &&fn)
+{
+    if (!layout_m) {
+        const double *p = buf + (long long)k * pitch + i;
+        d2q37::static_for<0, NPOP>([&](auto L) { fn(L, p + (long long)decltype(L)::value * plane); });
+        return;
+    }
+    int col[7];
+#pragma unroll
+    for (int d = -3; d <= 3; ++d) {
+        int c = i + d;
+        c += (c < 0) ? Lx : 0;
+        c -= (c >= Lx) ? Lx : 0;
+        col[d + 3] = c;
+    }
+    d2q37::static_for<0, NPOP>([&](auto L) {
+        constexpr int m = decltype(L)::value;
+        constexpr int mx = d2q37::pop_ex(m), mz = d2q37::pop_ez(m);
+        int q = k + mz;
+        if (q >= 0 && q < Lz) {                               // written by the even step of site (i, k) through an ordinary gather
+            fn(L, buf + (long long)(NPOP - 1 - m) * plane + (long long)q * pitch + col[mx + 3]);
+        } else {                                              // ... through a wall-reflected gather
+            q = q < 0 ? -1 - q : 2 * Lz - 1 - q;
+            fn(L, buf + (long long)d2q37::pop_index(-mx, mz) * plane + (long long)q * pitch + col[3 - mx]);
+        }
+    });
 }
 
 }  // namespace lbm

@@ -14,9 +14,13 @@
 // (R .. R+6) instead of R+6 for all -- 37 (R+3) row-populations instead of 37 (R+6), which is what makes room for
 // the stage.  Bottom wall (a3): three GHOST ring rows -3..-1 hold the velocity-reversed copy of rows 2..0 (the ghost
 // row picture of DESIGN.md reading 9), written by the producers of those rows, so the consumers' gather is uniform
-// there; at the top wall the mirror rows are still resident and the consumers remap indices.  Sites whose first-step
-// sources wrap (seam strips, a1) or reflect (wall rows) are gathered from global memory by their producer thread;
-// the TMA unit zero-fills those parts of the boxes and they are never read.
+// there; at the top wall the mirror rows are still resident and the consumers remap indices.  Periodic x (a1): every
+// row is stored with XH spare columns on either side, of which the nearest XW hold the periodic images (written by
+// the consumers of the seam strips, or refreshed by wrap_columns_kernel after any other writer), so the boxes of the
+// seam strips need no special case -- a per-thread global gather for the seam sites cost a factor of two on
+// single-wave launches (profiles/r2_two_step.md).  Sites whose first-step sources reflect (wall rows) are gathered
+// from global memory by their producer thread; the TMA unit zero-fills those parts of the boxes (rows outside the
+// lattice) and they are never read.
 // Arithmetic is raw_moments / kinetic_from_raw / equilibrium_blend of d2q37.cuh, i.e. exactly collide_site():
 // results are bit-identical to two launches of the one-step kernel (tested).
 //
@@ -64,6 +68,10 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+__device__ __forceinline__ void fence_proxy_async_smem()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
     unsigned done;
@@ -75,15 +83,16 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 
 template <int TX_, int R_, int NST_, int SL_>
 struct Step2sShape {
-    static constexpr int TX = TX_;                      // output columns per strip
-    static constexpr int W1 = TX_ + 6;                  // intermediate columns per strip
+    static constexpr int TX = TX_;                      // output columns per strip, at most (the launch picks w <= TX)
+    static constexpr int W1 = TX_ + 6;                  // intermediate columns per strip, at most
     static constexpr int CP = (TX_ + 6 + 1) / 2 * 2;    // ring row pitch (doubles)
     static constexpr int CW = (TX_ + 31) / 32 * 32;     // consumer threads per output row (whole warps)
     static constexpr int R = R_;                        // rows per pass
     static constexpr int NST = NST_;                    // stage buffers (passes of input in flight)
     static constexpr int SL = SL_;                      // ring slack: passes the producers may run ahead of the consumers
     static constexpr int NRB = SL_ + 1;                 // FULL / EMPTY barriers (pass i uses barrier i mod NRB)
-    static constexpr int NA = (R_ * (TX_ + 6) + 31) / 32;   // producer warps (one thread per intermediate site)
+    static constexpr int AW = (TX_ + 6 + 31) / 32 * 32;     // producer threads per intermediate row (whole warps)
+    static constexpr int NA = R_ * AW / 32;                 // producer warps (one thread per intermediate site)
     static constexpr int NB = R_ * CW / 32;                 // consumer warps (one thread per output site)
     static constexpr int NAT = NA * 32, NBT = NB * 32;
     static constexpr int NLT = 32;                          // one loader warp
@@ -106,6 +115,7 @@ struct Step2sShape {
     static constexpr size_t RING_DOUBLES = ((size_t)RING_ROWS * CP + 15) / 16 * 16;   // stage starts on a 128-byte line
     static constexpr size_t STAGE_DOUBLES = (size_t)NPOP * R_ * SP;   // per buffer
     static constexpr size_t SMEM = sizeof(double) * (RING_DOUBLES + NST_ * STAGE_DOUBLES);
+    static_assert((CW & (CW - 1)) == 0, "consumer lanes per row: a power of two");
     static_assert(R_ >= 1 && NST_ >= 1 && NST_ <= 4 && TX_ % 2 == 0 && XPAD <= SP - TX_ - 12, "shape");
     static_assert((R_ * SP * 8) % 128 == 0 && (RING_DOUBLES * 8) % 128 == 0, "TMA box destinations are 128-byte aligned");
 };
@@ -117,6 +127,8 @@ struct Step2sShape {
 //   <60,2,3,0> 15.7         (5 producer warps again)
 //   <64,2,1,1> 14.2, <64,3,1,0> 14.7   one stage buffer: the producers wait for the TMA round trip
 //   <112,1,2,0> 16.8, <120,1,1,0> 14.8  one row per pass, wide strips (5 % halo work instead of 11 %), fewer buffers
+//   <58,2,3,0> with the strip width a launch argument (round 2): 64 producer lanes per intermediate row, so no warp
+//                           straddles two rows; the host picks an even width <= 58 that divides Lx without a sliver
 #ifndef S2S_TX   // shape experiments: -DS2S_TX=.. -DS2S_R=.. -DS2S_NST=.. -DS2S_SL=..
 #define S2S_TX 56
 #define S2S_R 2
@@ -135,8 +147,9 @@ struct Step2sMaps {
 // Seven TMA box loads per pass, one per e_z: box = span of SP source columns from x0-6-XPAD (16-byte aligned in
 // global memory) x the R source rows (row - e_z) x the 3/5/7 populations with that e_z, written densely as
 // stage[l][row of the pass][span column]; the e_x shift is applied when the producers read the stage.  Coordinates
-// outside the lattice (periodic seam, walls) are zero-filled by the TMA unit and never read: the producer threads
-// whose sources wrap or reflect gather their site from global memory themselves (a1, a3).
+// outside the lattice (rows beyond the walls) are zero-filled by the TMA unit and never read: the producer threads
+// of wall rows gather their site from global memory themselves (a3); the periodic seam is covered by the wrap
+// columns (a1).
 // (Measured and dropped, profiles/r1_two_step.md: one 1-D bulk copy per row and population -- the TMA unit issues
 // ~1 copy per 63 cycles whatever its size, 7000 cycles per pass; per-thread 8-byte cp.async -- ~20 cycles of
 // L1TEX per warp instruction.)
@@ -161,27 +174,28 @@ __device__ __noinline__ void step2s_loader(const Step2sMaps *maps, double *stage
         __syncwarp();
         if (lane < 7) {
             const unsigned dst = st + (unsigned)((b * S::STAGE_DOUBLES + (size_t)l0 * S::R * S::SP) * 8);
+            // x coordinate in the tensor map, whose column 0 is stored column -XH (the wrap columns are part of the tensor)
             asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                         ::"r"(dst), "l"(map), "r"(x0 - 6 - S::XPAD), "r"(z0 - 3 + j * S::R - ez), "r"(l0), "r"(bar) : "memory");
+                         ::"r"(dst), "l"(map), "r"(x0 - 6 - S::XPAD + XH), "r"(z0 - 3 + j * S::R - ez), "r"(l0), "r"(bar) : "memory");
         }
         if (++b == S::NST) { b = 0; ++use; }
     }
 }
 
 // ---- producer warps: first step of intermediate rows z0-3 .. zend+2, R rows per pass ----
-template <class S>
+template <class S, bool ISO>
 __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, const double *stage, unsigned bar_full,
                                                 int tid, int x0, int z0, int ncols, int rlast, int NP)
 {
     // the four barrier arrays are consecutive (step2s_kernel): one base register
     const unsigned bar_empty = bar_full + 8 * S::NRB, bar_sfull = bar_empty + 8 * S::NRB, bar_sempty = bar_sfull + 8 * S::NST;
-    const int ar = tid / S::W1, aj = tid - ar * S::W1;
-    const bool a_lane = tid < S::R * S::W1 && aj < ncols + 6;
+    // AW lanes per intermediate row (whole warps, so that no warp straddles two rows of the stage or of the ring)
+    const int ar = tid / S::AW, aj = tid - ar * S::AW;
+    const bool a_lane = aj < ncols + 6;
     // stage [l][row of the pass][span column]; span column = aj + 3 + XPAD - e_lx
     const unsigned sp = (unsigned)__cvta_generic_to_shared(stage) + (unsigned)((ar * S::SP + aj + 3 + S::XPAD) * 8);
     const unsigned rp0 = (unsigned)__cvta_generic_to_shared(ring) + (unsigned)(aj * 8);   // ring column of this thread
     const int c = x0 - 3 + aj;                          // this thread's column, before the periodic wrap (a1)
-    const bool xwrap = c - 3 < 0 || c + 3 >= a.Lx;      // a source column wraps: the site is gathered from global memory
     int ac = c % a.Lx;
     if (ac < 0) ac += a.Lx;
     const int Lz = a.Lz;                                // kernel arguments into registers once (see the consumer)
@@ -194,10 +208,10 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
         const int row = z0 - 3 + j * S::R + ar;
         const bool v = a_lane && row >= 0 && row < rlast;
         double f[NPOP];
-        // sites whose sources wrap (seam strips) or reflect (wall rows, a3) bypass the stage; their loads are issued
-        // before the wait so that they overlap it
-        const bool gl = v && (xwrap || row < 3 || row >= Lz - 3);
-        if (gl) each_source_site<true>(a, ac, row, [&](auto L, const double *p) { f[decltype(L)::value] = ld_stream(p); });
+        // sites whose sources reflect (wall rows, a3) bypass the stage; their loads are issued before the wait so that
+        // they overlap it.  (Periodic x, a1, needs no such path: the boxes of the seam strips read the wrap columns.)
+        const bool gl = v && (row < 3 || row >= Lz - 3);
+        if (gl) each_source_site<true>(a, ac, row, [&](auto L, const double *p, bool) { f[decltype(L)::value] = ld_stream(p); });
         mbar_wait(bar_sfull + 8 * b, use & 1u);
         const unsigned sb = sp + (unsigned)(b * (S::STAGE_DOUBLES * 8));
         if (v && !gl) d2q37::static_for<0, NPOP>([&](auto L) {
@@ -210,12 +224,17 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
         // gathers of the same warp) -- a one-in-10^5-blocks error, profiles/r1_two_step.md.
         d2q37::RawMoments m;
         if (v) {
+            if (gl) wall_rows_adjust<ISO>(a, row, f);       // wall_kind 1: rows next to an isothermal wall (a3)
             m = d2q37::raw_moments(f);
             // keeps the arrive below the sums in the instruction stream: a DADD cannot issue before its operands
             // have returned from shared memory, and a warp issues in order (tests/test_library_cpu.py checks the
             // order in the SASS; making the barrier address depend on the sums instead costs 3.5 %)
             asm volatile("" : "+d"(m.m0), "+d"(m.jx), "+d"(m.jz), "+d"(m.m2));
         }
+        // generic-proxy reads of the stage -> async-proxy (TMA) rewrite of the same buffer: the arrive alone does not
+        // order across proxies, so the reads are fenced into the async proxy before the release (the pattern for
+        // generic reads of TMA-filled shared memory; the consume-before-release order above stays as a second guard)
+        fence_proxy_async_smem();
         mbar_arrive(bar_sempty + 8 * b);
         if (v) {
             const d2q37::Kinetic kin = d2q37::kinetic_from_raw(m);
@@ -257,13 +276,27 @@ __device__ __noinline__ void step2s_producer(const StepArgs &a, double *ring, co
 }
 
 // ---- consumer warps: second step of output rows z0 .. zend-1, R rows per pass ----
-template <class S>
+template <class S, bool ISO>
 __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ring, unsigned bar_full,
                                                 unsigned bar_empty, int bt, int x0, int z0, int ncols, int zend)
 {
     const int br = bt / S::CW, bj = bt - br * S::CW;
-    const bool b_lane = bj < ncols;
-    const unsigned q = (unsigned)__cvta_generic_to_shared(ring) + (unsigned)((bj + 3) * 8);   // ring column of this thread
+    // Periodic x (a1): the next launch's boxes read the wrap columns of THIS launch's destination copy (columns
+    // 0..XW-1 repeat after column Lx-1, columns Lx-XW..Lx-1 before column 0).  The CW - ncols spare lanes of a row
+    // write them: in the two seam strips a spare lane computes the same site as the lane that owns the seam column
+    // (same ring values, same arithmetic, same result) and stores it at the image position.  Only the starting values
+    // of two per-thread pointers differ, so the loop is untouched -- it has no register to spare: consumers that
+    // stored the image as a second store spilled and lost 10-25 %, a loader warp copying the columns (per-lane
+    // loads / stores, or TMA boxes) slowed the seam strips by 1.3-1.8x (profiles/r2_two_step.md).
+    int cj = bj, img = 0;                               // strip column this lane computes; offset of its store
+    bool b_lane = bj < ncols;
+    if (a.wrap_store) {
+        const bool lo = x0 == 0, hi = x0 + ncols == a.Lx;          // first / last strip (or both)
+        const int t = bj - ncols, th = t - (lo ? XW : 0);            // spare lane index; ... after the low seam's
+        if (lo && t >= 0 && t < XW) { cj = t; img = a.Lx; b_lane = true; }
+        else if (hi && th >= 0 && th < XW) { cj = ncols - XW + th; img = -a.Lx; b_lane = true; }
+    }
+    const unsigned q = (unsigned)__cvta_generic_to_shared(ring) + (unsigned)((cj + 3) * 8);   // ring column of this thread
     // kernel arguments into registers once: `a` is reached through a pointer here (non-inlined role), and every
     // global store would otherwise force its fields to be re-loaded.  Rows are counted relative to the chunk
     // (kq = k - z0) to keep the loop state small: the collision needs nearly all 168 registers.
@@ -271,7 +304,7 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
     const int lt = a.Lz - z0;                           // kq of the first row above the top wall
     const double omega = a.omega, gtau = a.gtau, dT = a.dT;
     const long long plane = a.plane;
-    double *p = a.dst + (long long)(z0 + br) * a.pitch + x0 + bj;    // this thread's site of the pass, population 0
+    double *p = a.dst + (long long)(z0 + br) * a.pitch + x0 + cj + img;    // this thread's site of the pass, population 0
     const long long pass_stride = (long long)S::R * a.pitch;
 
     for (int i = 0; i * S::R < zr; ++i, p += pass_stride) {
@@ -310,6 +343,8 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
         }
         d2q37::RawMoments m;                            // release the ring rows after the values were consumed (see the producer)
         if (bv) {
+            if constexpr (ISO)
+                if (kq + z0 < 3 || kq >= lt - 3) wall_rows_adjust<ISO>(a, kq + z0, f);
             m = d2q37::raw_moments(f);
             asm volatile("" : "+d"(m.m0), "+d"(m.jx), "+d"(m.jz), "+d"(m.m2));
         }
@@ -325,14 +360,15 @@ __device__ __noinline__ void step2s_consumer(const StepArgs &a, const double *ri
     }
 }
 
-template <class S>
+template <class S, bool ISO>
 __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_constant__ StepArgs a, const __grid_constant__ Step2sMaps maps, const int ZC)
 {
     extern __shared__ __align__(128) double smem2s[];    // ring [RING_ROWS][CP] | stage [NST][NPOP][R][SP]
     __shared__ unsigned long long bars[2 * S::NRB + 2 * S::NST];
     const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * S::TX, z0 = blockIdx.y * ZC;
-    const int ncols = min(S::TX, a.Lx - x0);            // output columns of this strip
+    const int w = a.w;                                   // strips of w <= TX columns (w even: TMA boxes start on 16 bytes)
+    const int x0 = blockIdx.x * w, z0 = blockIdx.y * ZC;
+    const int ncols = min(w, a.Lx - x0);                // output columns of this strip
     const int zend = min(a.Lz, z0 + ZC);                // output rows [z0, zend)
     const int rlast = min(a.Lz, zend + 3);              // intermediate rows [max(0, z0-3), rlast)
     const int NP = (zend - z0 + S::R - 1) / S::R;       // consumer passes
@@ -348,9 +384,9 @@ __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_cons
     __syncthreads();
     double *stage = smem2s + S::RING_DOUBLES;
     if (tid < S::NAT)
-        step2s_producer<S>(a, smem2s, stage, bar_full, tid, x0, z0, ncols, rlast, NP);
+        step2s_producer<S, ISO>(a, smem2s, stage, bar_full, tid, x0, z0, ncols, rlast, NP);
     else if (tid < S::NAT + S::NBT)
-        step2s_consumer<S>(a, smem2s, bar_full, bar_empty, tid - S::NAT, x0, z0, ncols, zend);
+        step2s_consumer<S, ISO>(a, smem2s, bar_full, bar_empty, tid - S::NAT, x0, z0, ncols, zend);
     else
         step2s_loader<S>(&maps, stage, bar_sfull, bar_sempty, tid - S::NAT - S::NBT, x0, z0, NP);
 }

@@ -8,7 +8,7 @@ import pytest
 import synthetic_inputs as si
 
 pytestmark = pytest.mark.gpu
-NSTEPS = 3
+NSTEPS = 7          # three fused launches of the two-step kernel and one single step
 M = 3 * NSTEPS      # rows/columns near a window edge that see outside the window
 
 
@@ -29,17 +29,31 @@ def _window(dense, r0, r1, cols):
     return dense[:, r0:r1][:, :, cols].contiguous().cpu().numpy()
 
 
-def _check_windows(orc, before, after, Lx, Lz, tau, g, tol):
-    """before/after: dense device populations [37][Lz][Lx] at step 0 and step NSTEPS."""
+def _check_windows(orc, before, after, Lx, Lz, tau, g, tol, plan=None):
+    """before/after: dense device populations [37][Lz][Lx] at step 0 and step NSTEPS.  With `plan` = (fused, strip
+    width w, rows per chunk ZC) of the launch, extra windows straddle a chunk boundary (rows around c ZC, where one
+    block hands over to the next: ring wrap, warm-up rows) and a strip boundary (columns around s w)."""
     import torch
-    W = 40
+    W = 40 + 2 * M
     worst = 0.0
     cases = [  # (first row, first column, kind)
-        (0, Lx - 17, "bottom"),                 # bottom wall, straddles the periodic seam
+        (0, Lx - W // 2 - 1, "bottom"),         # bottom wall, straddles the periodic seam
         (Lz - W, Lx // 2 + 5, "top"),           # top wall
         (Lz // 2 - W // 2, 3, "bulk"),          # the interface region
-        (Lz - W - 1000, Lx - 23, "bulk"),       # far rows, seam
+        (Lz - W - 1000, Lx - W // 2 - 3, "bulk"),   # far rows, seam
     ]
+    if plan is not None and plan[0]:
+        _, w, zc = plan
+        nchunks, nstrips = (Lz + zc - 1) // zc, (Lx + w - 1) // w
+        assert nstrips >= 3
+        sx = (nstrips // 2) * w                  # a strip boundary in the middle of the lattice
+        cases.append((Lz // 3, sx - W // 2, "bulk"))                     # a strip boundary
+        if nchunks >= 2:
+            cases += [
+                (zc - W // 2, sx - W // 2, "bulk"),                          # first chunk boundary x strip boundary
+                ((nchunks // 2) * zc - W // 2, sx - W // 2 + 11, "bulk"),    # a middle chunk boundary
+                ((nchunks - 1) * zc - W // 2, Lx - W // 2, "bulk"),          # last chunk boundary on the seam
+            ]
     for r0, c0, kind in cases:
         cols = (torch.arange(c0, c0 + W, device=before.device) % Lx)
         w0 = _window(before, r0, r0 + W, cols)
@@ -56,12 +70,14 @@ def test_config4_fullsize_sampled_windows_and_conservation(pkg, orc):
     """BASELINE.json configs[3] exactly as bench.py launches it."""
     cfg = si.rt_config(4)
     lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    plan = lat.plan()
+    assert plan[0] and plan[2] < cfg.Lz                      # the bench's launch: the two-step kernel, several chunks
     lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
     t0 = lat.totals()
     before = lat.get_populations()
     lat.step(NSTEPS)
     after = lat.get_populations()
-    _check_windows(orc, before, after, cfg.Lx, cfg.Lz, cfg.tau, cfg.g, 1e-13)
+    _check_windows(orc, before, after, cfg.Lx, cfg.Lz, cfg.tau, cfg.g, 1e-13, plan)
     del before, after
     lat.step(50 - NSTEPS)
     t1 = lat.totals()
@@ -89,9 +105,10 @@ def test_largest_sweep_lattice_offsets_beyond_32_bits(pkg, orc):
     got0 = _window(before, r0, r0 + W, torch.arange(c0, c0 + W, device="cuda"))
     assert float(np.max(np.abs(got0 - ref0) / ref0)) < 1e-13
     del fields
+    plan = lat.plan()
     lat.step(NSTEPS)
     after = lat.get_populations()
-    _check_windows(orc, before, after, Lx, Lz, si.SWEEP_TAU, si.SWEEP_G, 1e-13)
+    _check_windows(orc, before, after, Lx, Lz, si.SWEEP_TAU, si.SWEEP_G, 1e-13, plan)
     lat.close()
 
 
@@ -110,6 +127,61 @@ def test_two_step_kernel_back_to_back_launches_stay_bitwise_equal(pkg):
     for lat in (a, b):
         lat.init_equilibrium(*fields)
         lat.step(200)
-    assert b.kernel_launches - l0 == 1 + 100          # init + 100 two-step launches: the default path is the fused one
+    assert b.kernel_launches - l0 == 1 + 1 + 100      # init + wrap-column refresh + 100 two-step launches: the default path is the fused one
+    assert torch.equal(a.get_populations(), b.get_populations())
+    a.close(); b.close()
+
+
+def test_config3_100_steps_slabs_against_oracle(pkg, orc):
+    """BASELINE.json configs[2]: 2048x4096 double front, white-noise interfaces, tau = 0.7, the automatic launch plan,
+    100 steps (the north_star criterion).  The domain of dependence of a row after n steps is +-3n rows, so the
+    oracle steps full-width slabs (exact periodic x, seam included) of h + 2 x 300 rows and the central h rows are
+    compared population by population: one slab per interface, one on the bottom wall, one on the top wall."""
+    cfg = si.rt_config(3)
+    n, h = 100, 24
+    halo = 3 * n
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    assert lat.plan()[0]
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    before = lat.get_populations()
+    lat.step(n)
+    after = lat.get_populations()
+    lat.close()
+    lo_if, hi_if = int(cfg.Lz / 2 - cfg.delta / 2), int(cfg.Lz / 2 + cfg.delta / 2)
+    worst = 0.0
+    for kind, centre in (("bulk", lo_if), ("bulk", hi_if), ("bottom", 0), ("top", cfg.Lz)):
+        if kind == "bulk":
+            r0, r1 = centre - h // 2 - halo, centre + h // 2 + halo
+            rows = slice(halo, halo + h)
+        elif kind == "bottom":
+            r0, r1 = 0, h + halo
+            rows = slice(0, h)
+        else:
+            r0, r1 = cfg.Lz - h - halo, cfg.Lz
+            rows = slice(halo, halo + h)
+        w0 = before[:, r0:r1].contiguous().cpu().numpy()
+        w1 = after[:, r0:r1].contiguous().cpu().numpy()
+        # bulk slabs: periodic in z (the contamination from the wrong closure stays within `halo` rows of the edges);
+        # wall slabs: the real wall on one side, a spurious wall on the other, `halo` rows away from the rows compared
+        ref = orc.step(w0, cfg.tau, cfg.g, nsteps=n, periodic_z=(kind == "bulk"))
+        a, b = w1[:, rows], ref[:, rows]
+        worst = max(worst, float(np.max(np.abs(a - b) / np.abs(b))))
+        del w0, w1, ref
+    assert worst < 1e-11, worst
+
+
+def test_two_step_kernel_bitwise_at_the_large_lattice_plan(pkg):
+    """The two-step kernel in the launch plan of the large lattices (a few long chunks per strip, whole waves) against
+    the one-step kernel, 50 steps at 2048x4096, every population of every site, bit for bit."""
+    import torch
+    Lx, Lz = 2048, 4096
+    fields = si.sweep_fields_torch(Lx, Lz, si.DEFAULT_SEED, "cuda")
+    a, b = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G), pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G)
+    a.set_variant(1)
+    fused, w, zc = b.plan()
+    assert fused and zc >= 128
+    for lat in (a, b):
+        lat.init_equilibrium(*fields)
+        lat.step(50)
     assert torch.equal(a.get_populations(), b.get_populations())
     a.close(); b.close()

@@ -67,6 +67,28 @@ def test_config1_100_steps_population_parity(pkg, orc, variant):
     lat.close()
 
 
+def test_config2_100_steps_population_parity_automatic_plan(pkg, orc):
+    """BASELINE.json configs[1] in full: 512x1024 double-front RT, 16 modes, seed 12345, the AUTOMATIC launch plan
+    (the two-step kernel with many short chunks at this size), 100 steps: every population of every site, the
+    lattice totals and the mixing widths L_u, L_d against the oracle."""
+    cfg = si.rt_config(2)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    fused, w, zc = lat.plan()
+    assert fused and w < cfg.Lx and zc < cfg.Lz              # several strips and several chunks per strip
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    lat.step(100)
+    got = lat.get_populations(host=True).numpy()
+    _, ref = _oracle_rt(orc, cfg, si.DEFAULT_SEED, 100)
+    assert _rel(got, ref) < POP_RTOL
+    tg, tr = lat.totals(), orc.totals(ref)
+    assert abs(tg[0] / tr[0] - 1) < TOT_RTOL and abs(tg[3] / tr[3] - 1) < TOT_RTOL
+    assert abs(tg[1] - tr[1]) < TOT_RTOL * tr[0] and abs(tg[2] - tr[2]) < TOT_RTOL * tr[0]
+    lu, ld, tbar = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u)
+    olu, old, otbar = orc.mixing_widths(ref, cfg.g, cfg.T_d, cfg.T_m, cfg.T_u)
+    assert np.max(np.abs(tbar - otbar)) < 1e-13 and abs(lu - olu) < 1e-10 and abs(ld - old) < 1e-10
+    lat.close()
+
+
 @pytest.mark.parametrize("variant", [0, 3])
 @pytest.mark.parametrize("Lx,Lz,steps", [(7, 6, 5), (33, 9, 12), (130, 70, 20), (257, 40, 10), (520, 18, 7)])
 def test_ragged_and_tiny_lattices_from_identical_populations(pkg, orc, Lx, Lz, steps, variant):

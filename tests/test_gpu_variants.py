@@ -1,0 +1,248 @@
+"""GPU parity for the SURVEY 8(f) rows: isothermal no-slip walls (wall_kind 1, reading 19), in-place streaming with
+one lattice copy, z-slabs with exchanged ghost rows -- each against the CPU oracle element by element (1e-11) and,
+where the arithmetic is the same, bit for bit against the two-copy whole-lattice path.  Run on the B200 box."""
+import numpy as np
+import pytest
+
+import synthetic_inputs as si
+
+pytestmark = pytest.mark.gpu
+POP_RTOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import __graft_entry__ as g
+    g.build()
+    import paper_1405_1253_b200 as p
+    return p
+
+
+def _rel(a, b):
+    return float(np.max(np.abs(a - b) / np.abs(b)))
+
+
+def _random_state(orc, Lx, Lz, seed):
+    rng = np.random.default_rng(seed)
+    rho = 1 + 0.05 * rng.uniform(-1, 1, (Lz, Lx)); T = 1 + 0.05 * rng.uniform(-1, 1, (Lz, Lx))
+    ux = 0.03 * rng.uniform(-1, 1, (Lz, Lx)); uz = 0.03 * rng.uniform(-1, 1, (Lz, Lx))
+    return orc.init_equilibrium(rho, ux, uz, T) * (1 + 0.01 * rng.uniform(-1, 1, (37, Lz, Lx)))
+
+
+# ------------------------------------------------------------------------------------------ isothermal walls
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+def test_isothermal_walls_config1_100_steps(pkg, orc, variant):
+    """BASELINE.json configs[0] with wall_kind 1 (walls at T_d below, T_u above): 100 steps, all populations."""
+    cfg = si.rt_config(1)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, wall_kind=1, T_wall=(cfg.T_d, cfg.T_u))
+    lat.set_variant(variant)
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    lat.step(100)
+    got = lat.get_populations(host=True).numpy()
+    f0 = orc.init_rt(cfg.Lx, cfg.Lz, cfg.g, si.DEFAULT_SEED, **cfg.rt_args())
+    ref = orc.step(f0, cfg.tau, cfg.g, nsteps=100, wall_kind=1, T_bot=cfg.T_d, T_top=cfg.T_u)
+    assert _rel(got, ref) < POP_RTOL
+    assert _rel(got, orc.step(f0, cfg.tau, cfg.g, nsteps=100)) > 1e-6        # and it is not the bounce-back result
+    _, ux, uz, T = [x.cpu().numpy() for x in lat.moments()]
+    assert np.abs(uz[:3]).max() < 1e-15 and np.abs(T[:3] - cfg.T_d).max() < 1e-14 and np.abs(T[-3:] - cfg.T_u).max() < 1e-14
+    tg, tr = lat.totals(), orc.totals(ref)
+    assert abs(tg[0] / tr[0] - 1) < 1e-12 and abs(tg[3] / tr[3] - 1) < 1e-12
+    lat.close()
+
+
+@pytest.mark.parametrize("Lx,Lz,zchunk,n", [(7, 6, 3, 4), (33, 9, 3, 5), (130, 70, 9, 7), (257, 40, 15, 4), (300, 100, 28, 12)])
+def test_isothermal_walls_two_step_kernel_ragged(pkg, orc, Lx, Lz, zchunk, n):
+    """wall_kind 1 in the two-step kernel (producer wall rows of the first step, consumer wall rows of the second):
+    lattices made only of wall rows, ragged strips, chunk tails; bitwise equal to the one-step kernel, and within
+    the oracle tolerance."""
+    import torch
+    f0 = _random_state(orc, Lx, Lz, Lx * 7 + Lz)
+    a = pkg.Lattice(Lx, Lz, 0.66, 3e-4, wall_kind=1, T_wall=(1.03, 0.96))
+    b = pkg.Lattice(Lx, Lz, 0.66, 3e-4, wall_kind=1, T_wall=(1.03, 0.96))
+    a.set_variant(1); b.set_variant(3); b.set_zchunk(zchunk)
+    for lat in (a, b):
+        lat.set_populations(torch.from_numpy(f0).cuda())
+        lat.step(n)
+    assert torch.equal(a.get_populations(), b.get_populations())
+    ref = orc.step(f0, 0.66, 3e-4, nsteps=n, wall_kind=1, T_bot=1.03, T_top=0.96)
+    assert _rel(b.get_populations(host=True).numpy(), ref) < POP_RTOL
+    a.close(); b.close()
+
+
+# ------------------------------------------------------------------------------------------ in-place streaming
+@pytest.mark.parametrize("wall_kind", [0, 1])
+@pytest.mark.parametrize("Lx,Lz", [(7, 6), (33, 9), (130, 70), (257, 40)])
+def test_inplace_streaming_matches_oracle_after_every_step(pkg, orc, Lx, Lz, wall_kind):
+    """One lattice copy: after an odd number of steps the store is in the shifted layout, after an even number in
+    the ordinary one; lbm_get_populations, lbm_moments and the row diagnostics read either.  Every step 1..6 against
+    the oracle, and bit for bit against the two-copy path."""
+    import torch
+    f0 = _random_state(orc, Lx, Lz, Lx + 13 * Lz)
+    kw = dict(wall_kind=wall_kind, T_wall=(1.02, 0.97))
+    one, two = pkg.Lattice(Lx, Lz, 0.7, 2e-4, inplace=True, **kw), pkg.Lattice(Lx, Lz, 0.7, 2e-4, **kw)
+    two.set_variant(1)
+    for lat in (one, two):
+        lat.set_populations(torch.from_numpy(f0).cuda())
+    ref = f0
+    for n in range(1, 7):
+        one.step(1); two.step(1)
+        ref = orc.step(ref, 0.7, 2e-4, nsteps=1, wall_kind=wall_kind, T_bot=1.02, T_top=0.97)
+        got = one.get_populations()
+        assert torch.equal(got, two.get_populations()), n
+        assert _rel(got.cpu().numpy(), ref) < POP_RTOL
+        assert np.array_equal(one.get_populations(host=True).numpy(), got.cpu().numpy())     # plane-by-plane host path
+        for x, y in zip(one.moments(), two.moments()):
+            assert torch.equal(x, y)
+        assert np.array_equal(one.totals(), two.totals())
+    with pytest.raises(pkg.LbmError):
+        one.set_variant(3); one.step(2)                      # the two-step kernel needs two copies
+    one.close(); two.close()
+
+
+def test_inplace_streaming_config1_100_steps_and_host_upload(pkg, orc):
+    cfg = si.rt_config(1)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, inplace=True)
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    lat.step(99)                                              # ends in the shifted layout
+    f0 = orc.init_rt(cfg.Lx, cfg.Lz, cfg.g, si.DEFAULT_SEED, **cfg.rt_args())
+    assert _rel(lat.get_populations(host=True).numpy(), orc.step(f0, cfg.tau, cfg.g, nsteps=99)) < POP_RTOL
+    lu, ld, tbar = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u)
+    olu, old, otbar = orc.mixing_widths(orc.step(f0, cfg.tau, cfg.g, nsteps=99), cfg.g, cfg.T_d, cfg.T_m, cfg.T_u)
+    assert np.max(np.abs(tbar - otbar)) < 1e-13 and abs(lu - olu) < 1e-10 and abs(ld - old) < 1e-10
+    import torch
+    lat.set_populations(torch.from_numpy(f0))                 # host upload resets to the ordinary layout
+    lat.step(2)
+    assert _rel(lat.get_populations(host=True).numpy(), orc.step(f0, cfg.tau, cfg.g, nsteps=2)) < POP_RTOL
+    lat.close()
+
+
+# ------------------------------------------------------------------------------------------ z-slabs
+def _run_slabs(pkg, slabs, nsteps, exchange_stream=None):
+    """Steps slabs that live on one device: messages are packed on the exchange stream, copied device to device and
+    unpacked there while the interior rows run on the main stream (the exchange hides behind the
+    bulk), then the edge rows."""
+    import torch
+    main = torch.cuda.current_stream()
+    xs = exchange_stream or torch.cuda.Stream()
+    up = [s.new_message() for s in slabs]      # message of slab i to the slab above
+    dn = [s.new_message() for s in slabs]
+    for _ in range(nsteps):
+        xs.wait_stream(main)
+        for i, s in enumerate(slabs):
+            if s.open_above: s.pack(1, up[i], stream=xs)
+            if s.open_below: s.pack(0, dn[i], stream=xs)
+        for s in slabs:
+            s.step_part(pkg.Slab.INTERIOR, stream=main)
+        for i, s in enumerate(slabs):                         # "transport": the neighbour's message, same device here
+            if s.open_below: s.unpack(0, up[i - 1], stream=xs)
+            if s.open_above: s.unpack(1, dn[i + 1], stream=xs)
+        main.wait_stream(xs)
+        for s in slabs:
+            s.step_part(pkg.Slab.EDGES, stream=main)
+    torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("wall_kind", [0, 1])
+@pytest.mark.parametrize("Lx,Lz,cuts,n", [(64, 128, (0, 50, 128), 100), (130, 70, (0, 6, 30, 64, 70), 25), (33, 40, (0, 17, 40), 9)])
+def test_slabs_with_exchanged_ghost_rows_equal_the_whole_lattice(pkg, orc, Lx, Lz, cuts, n, wall_kind):
+    """The lattice cut into z-slabs (down to the minimum of 6 rows), 26 population-rows exchanged per open side and
+    step: bit-identical to the whole-lattice run, and within the oracle tolerance."""
+    import torch
+    f0 = _random_state(orc, Lx, Lz, 5 * Lx + Lz)
+    kw = dict(wall_kind=wall_kind, T_wall=(1.02, 0.97))
+    whole = pkg.Lattice(Lx, Lz, 0.75, 2e-4, **kw)
+    whole.set_variant(1)
+    whole.set_populations(torch.from_numpy(f0).cuda())
+    whole.step(n)
+    slabs = [pkg.Slab(Lx, Lz, z0, z1 - z0, 0.75, 2e-4, **kw) for z0, z1 in zip(cuts[:-1], cuts[1:])]
+    for s in slabs:
+        s.set_populations(torch.from_numpy(np.ascontiguousarray(f0[:, s.z0:s.z0 + s.nz])).cuda())
+    _run_slabs(pkg, slabs, n)
+    got = torch.cat([s.get_populations() for s in slabs], dim=1)
+    assert torch.equal(got, whole.get_populations())
+    ref = orc.step(f0, 0.75, 2e-4, nsteps=n, wall_kind=wall_kind, T_bot=1.02, T_top=0.97)
+    assert _rel(got.cpu().numpy(), ref) < POP_RTOL
+    assert abs(sum(s.totals()[0] for s in slabs) / whole.totals()[0] - 1) < 1e-14       # partial sums add up
+    with pytest.raises(pkg.LbmError):
+        slabs[0].pack(0, slabs[0].new_message())                                          # side 0 of the bottom slab is a wall
+    with pytest.raises(pkg.LbmError):
+        slabs[0].step_part(pkg.Slab.EDGES)                                                # interior first
+    for s in slabs:
+        s.close()
+    whole.close()
+
+
+def test_slabs_rt_config_init_and_widths(pkg, orc):
+    """lbm_init_rt on slabs uses global heights and fills the ghost rows; the mixing widths are partial sums."""
+    cfg = si.scaled(si.rt_config(2), 128, 256)
+    whole = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    whole.set_variant(1)
+    whole.init_rt(7, **cfg.rt_args())
+    slabs = [pkg.Slab(cfg.Lx, cfg.Lz, z0, nz, cfg.tau, cfg.g) for z0, nz in ((0, 100), (100, 60), (160, 96))]
+    for s in slabs:
+        s.init_rt(7, **cfg.rt_args())
+    import torch
+    assert torch.equal(torch.cat([s.get_populations() for s in slabs], dim=1), whole.get_populations())
+    whole.step(40)
+    _run_slabs(pkg, slabs, 40)
+    assert torch.equal(torch.cat([s.get_populations() for s in slabs], dim=1), whole.get_populations())
+    lu, ld, tbar = whole.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u)
+    parts = [s.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u) for s in slabs]
+    assert abs(sum(p[0] for p in parts) - lu) < 1e-12 and abs(sum(p[1] for p in parts) - ld) < 1e-12
+    assert np.array_equal(np.concatenate([p[2] for p in parts]), tbar)
+    for s in slabs:
+        s.close()
+    whole.close()
+
+
+# ------------------------------------------------------------------------------------------ boundary behaviour
+def test_fused_diagnostics_equal_the_single_calls_and_null_moments_are_rejected(pkg):
+    cfg = si.scaled(si.rt_config(2), 200, 96)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    lat.init_rt(5, **cfg.rt_args())
+    lat.step(20)
+    d = lat.diagnostics(cfg.T_d, cfg.T_m, cfg.T_u)
+    lu, ld, tbar = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u)
+    prof = lat.profiles()
+    assert d["L_u"] == lu and d["L_d"] == ld and np.array_equal(d["totals"], lat.totals())
+    for key, want in zip(("Tbar", "Trms", "Ekbar", "Ekrms"), prof):
+        assert np.array_equal(d[key], want)
+    assert np.array_equal(tbar, prof[0])
+    l0 = lat.kernel_launches
+    lat.diagnostics(cfg.T_d, cfg.T_m, cfg.T_u)
+    assert lat.kernel_launches - l0 == 2                      # one pass over the lattice + one small block
+    with pytest.raises(pkg.LbmError):
+        lat.moments(alloc=False)                              # all four outputs null
+    at, tau_rt = pkg.rt_scales(cfg.Lx, cfg.g, cfg.T_d, cfg.T_u)
+    assert abs(at - (cfg.T_d - cfg.T_u) / (cfg.T_d + cfg.T_u)) < 1e-16 and abs(tau_rt - (cfg.Lx / (cfg.g * at)) ** 0.5) < 1e-9
+    lat.close()
+
+
+def test_graph_capture_of_the_two_step_kernel_and_odd_launch_counts(pkg):
+    """lbm_step under stream capture on a lattice that takes the fused path (tensor maps as __grid_constant__
+    kernel arguments, the shared-memory opt-in): 4 steps = 2 launches are captured and replayed; 2 steps = 1 launch
+    would leave the other copy current and are rejected, as are 3 one-step launches."""
+    import torch
+    Lx, Lz = 512, 1024
+    fields = [x for x in si.sweep_fields_torch(Lx, Lz, 4, "cuda")]
+    a, b = pkg.Lattice(Lx, Lz, 0.8, 1e-4), pkg.Lattice(Lx, Lz, 0.8, 1e-4)
+    assert b.plan()[0]
+    a.init_equilibrium(*fields); b.init_equilibrium(*fields)
+    a.step(4 + 3 * 4)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        b.step(4, stream=s)                                   # warm-up outside capture
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            b.step(4, stream=s)
+            with pytest.raises(pkg.LbmError):
+                b.step(2, stream=s)                           # one fused launch: odd
+        for _ in range(3):
+            graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(a.get_populations(), b.get_populations())
+    a.close(); b.close()
