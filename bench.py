@@ -367,6 +367,61 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slabs(args):
+    """--slabs under torchrun (N > 1): ONE lattice (the N = 1 workload) cut into z-slabs, one per rank, 26
+    population-rows exchanged per open side and step over NCCL, hidden behind the interior rows (SURVEY 8(f)4;
+    PAPER.md:110, 116-118).  Strong scaling: value = sites x steps / max-over-ranks time.  Not the default N > 1 mode
+    (north_star fixes one GPU: the default is independent replicas); unmeasured on hardware in this run (one GPU per
+    call), verified on one GPU by tests/test_gpu_variants.py (slabs on one device, bit-identical to the whole lattice)."""
+    import torch
+    import torch.distributed as dist
+
+    import __graft_entry__ as entry
+    from paper_1405_1253_b200.slab_ring import SlabRing
+
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    if world < 2:
+        raise SystemExit("bench.py --slabs needs torchrun with N > 1 ranks")
+    torch.cuda.set_device(local)
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        entry.build()
+    dist.barrier()
+    cfg = si.rt_config(args.config)
+    ring = SlabRing(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, rank, world)
+    ring.slab.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize(); dist.barrier(); torch.cuda.synchronize()
+
+    ring.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local); sampler.start()
+    l0 = ring.slab.kernel_launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream); ring.step(args.steps); e1.record(stream)
+    barrier()
+    clocks = sampler.finish()
+    t = reduce_max([e0.elapsed_time(e1) * 1e-3], world, "cuda")[0]
+    part = ring.slab.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)
+    w = torch.tensor([part[0], part[1]], dtype=torch.float64, device="cuda")
+    dist.all_reduce(w)                                           # the widths of eq. 12 are sums over rows
+    launches = ring.slab.kernel_launches - l0
+    if rank == 0:
+        sites = cfg.Lx * cfg.Lz
+        print(json.dumps({
+            "metric": "MLUPS (FP64)", "value": sites * args.steps / t / 1e6, "unit": "MLUPS", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "Lx": cfg.Lx, "Lz": cfg.Lz, "tau": cfg.tau, "g": cfg.g,
+                       "parallelism": f"{world} z-slabs, 3 ghost rows per open side, 26 population-rows per message",
+                       "message_bytes": 26 * cfg.Lx * 8, "L_u": float(w[0]), "L_d": float(w[1])},
+            "gpu_launches": launches, "clocks": clocks}))
+    ring.close()
+    dist.destroy_process_group()
+
+
 def run_sweep(args):
     """--sweep: BASELINE.json configs[4] -- steady-state throughput from 256x512 to 8192x16384, populations at
     the equilibrium of i.i.d. rho, T, u fields; 200 timed steps per size (after 10 warm-up), one JSON line per
@@ -385,7 +440,7 @@ def run_sweep(args):
     for Lx, Lz in sizes:
         sites = Lx * Lz
         fields = si.sweep_fields_torch(Lx, Lz, si.DEFAULT_SEED, "cuda")
-        lat = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G)
+        lat = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G, inplace=args.inplace)
         for v in variants:
             lat.set_variant(v)
             if args.zchunk:
@@ -400,7 +455,7 @@ def run_sweep(args):
             t = e0.elapsed_time(e1) * 1e-3 / args.steps
             tm = e1.elapsed_time(e2) * 1e-3
             tot = lat.totals()
-            print(json.dumps({"sweep": f"{Lx}x{Lz}", "variant": v, "zchunk": args.zchunk, "mlups": sites / t / 1e6, "us_per_step": t * 1e6,
+            print(json.dumps({"sweep": f"{Lx}x{Lz}", "variant": v, "inplace": args.inplace, "plan": lat.plan(), "zchunk": args.zchunk, "mlups": sites / t / 1e6, "us_per_step": t * 1e6,
                               "gbs": BYTES_PER_SITE * sites / t / 1e9, "frac_of_measured_peak": BYTES_PER_SITE * sites / t / 1e9 / peak,
                               "resident": "L2" if 2 * 37 * 8 * sites < 126e6 else "HBM",
                               "moments_gbs": 328 * sites / tm / 1e9, "mass": tot[0]}), flush=True)
@@ -428,12 +483,16 @@ def main():
                     help="seconds of the extra sustained-throughput leg after the timed region (0 = skip)")
     ap.add_argument("--sweep", action="store_true", help="config 5: throughput sweep over lattice sizes")
     ap.add_argument("--sweep-variants", default="0")
+    ap.add_argument("--inplace", action="store_true", help="sweep with ONE lattice copy (in-place streaming)")
+    ap.add_argument("--slabs", action="store_true", help="N > 1: one lattice cut into z-slabs over the ranks (strong scaling)")
     ap.add_argument("--sweep-sizes", default="", help="e.g. 256x512,4096x8192 (default: all of config 5)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
     if args.sweep:
         run_sweep(args)
+    elif args.slabs:
+        run_slabs(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -130,6 +130,10 @@ int lbm_init_equilibrium(lbm_t *h, const double *rho, const double *ux, const do
 int lbm_set_populations(lbm_t *h, const double *f_dev, void *stream);
 int lbm_get_populations(lbm_t *h, double *f_dev, void *stream);
 int lbm_set_populations_host(lbm_t *h, const double *f_host, void *stream);
+/* A window of the stored populations, dense [37][nk][ni] into the DEVICE array f_dev: rows k0 .. k0+nk-1, columns
+ * i0 .. i0+ni-1 taken modulo Lx (a window may straddle the periodic seam).  For lattices whose whole dense array
+ * does not fit beside the lattice (16384 x 16384 in place).  Asynchronous.  Errors: rows outside [0, Lz), ni > Lx. */
+int lbm_get_window(lbm_t *h, int k0, int nk, int i0, int ni, double *f_dev, void *stream);
 int lbm_get_populations_host(lbm_t *h, double *f_host, void *stream);
 
 /* Enqueues n x (propagate + bc + collide) on `stream`; asynchronous.  Afterwards the

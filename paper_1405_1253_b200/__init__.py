@@ -148,6 +148,15 @@ class Lattice:
         binding.check(fn(self._h, _dptr(out), _stream_ptr(stream, self.device)))
         return out
 
+    @_on_device
+    def get_window(self, k0: int, nk: int, i0: int, ni: int, stream=None):
+        """Dense [37][nk][ni] populations of rows k0.., columns i0.. (mod Lx) (lbm_get_window)."""
+        import torch
+        out = torch.empty((NPOP, nk, ni), dtype=torch.float64, device=self.device)
+        binding.check(self._lib.lbm_get_window(self._h, int(k0), int(nk), int(i0), int(ni), _dptr(out),
+                                               _stream_ptr(stream, self.device)))
+        return out
+
     # ---- the hot path
     @_on_device
     def step(self, n: int = 1, stream=None):

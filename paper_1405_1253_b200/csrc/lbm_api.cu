@@ -139,6 +139,8 @@ struct lbm_handle {
     lbm::Step2sMaps maps[2];
     double *scratch;       // device: row diagnostics [8][nz] | results[8] | h_lo[Lx] | h_hi[Lx]
     double *stage[4];      // device staging fields for lbm_run_host (lazy)
+    int persist_tb, persist_blocks;   // persistent small-lattice kernel: block size and grid (0 = not applicable)
+    unsigned *d_counter;   // device: grid-barrier counter of the persistent kernel
     double *plane_stage;   // device staging of one dense population plane for the _host copies of in-place handles (lazy)
     lbm::Layout layout() const { return lbm::Layout{Lx, Lz, pitch, plane, glo, nz, layout_m}; }
     double *d_rows() const { return scratch; }
@@ -323,6 +325,7 @@ int create_common(lbm_t **out, int Lx, int rows_stored, const lbm_params *p, con
     h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 0; h->scratch = nullptr; h->plane_stage = nullptr;
     h->plan = lbm_plan{};
     h->tma_ok = false;
+    h->persist_tb = h->persist_blocks = 0; h->d_counter = nullptr;
     for (auto &s : h->stage) s = nullptr;
     *out = h;
     return LBM_OK;
@@ -341,6 +344,23 @@ int finish_create(lbm_t **out)
             cudaGetLastError();
             h->tma_ok = false;
         }
+    }
+    // Small lattices (one site per co-resident thread): lbm_step(n) is one cooperative launch of the persistent kernel
+    if (!h->inplace && !h->slab) {
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->dev);
+        const long long sites = (long long)h->Lx * h->Lz;
+        const int tb = sites <= 64LL * h->sm_count ? 64 : 128;       // spread a tiny lattice over all SMs
+        const long long blocks = (sites + tb - 1) / tb;
+        int per_sm = 0;
+        cudaError_t eo = tb == 64 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lbm::step_persistent_kernel<64, false>, 64, 0)
+                                  : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lbm::step_persistent_kernel<128, false>, 128, 0);
+        if (coop && eo == cudaSuccess && blocks <= (long long)per_sm * h->sm_count && blocks <= 2LL * h->sm_count &&
+            cudaMalloc(&h->d_counter, sizeof(unsigned)) == cudaSuccess) {
+            h->persist_tb = tb;
+            h->persist_blocks = (int)blocks;
+        }
+        cudaGetLastError();
     }
     cudaError_t e = cudaMalloc(&h->scratch, sizeof(double) * (8LL * h->nz + 8 + 2LL * h->Lx));
     if (e != cudaSuccess) {
@@ -428,6 +448,7 @@ int lbm_destroy(lbm_t *h)
 {
     if (!h) return LBM_OK;
     cudaFree(h->scratch);
+    cudaFree(h->d_counter);
     cudaFree(h->plane_stage);
     for (auto s : h->stage) cudaFree(s);
     delete h;
@@ -489,6 +510,18 @@ int lbm_get_populations(lbm_t *h, double *f_dev, void *stream)
     if (!f_dev) return fail(LBM_ERR_INVALID, "lbm_get_populations: null pointer");
     dim3 grid((h->Lx + lbm::AUX_TX - 1) / lbm::AUX_TX, h->nz, LBM_NPOP);
     lbm::unpack_kernel<<<grid, lbm::AUX_TX, 0, (cudaStream_t)stream>>>(h->buf[h->cur], h->layout(), f_dev, 0);
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
+int lbm_get_window(lbm_t *h, int k0, int nk, int i0, int ni, double *f_dev, void *stream)
+{
+    NEED(h);
+    if (!f_dev) return fail(LBM_ERR_INVALID, "lbm_get_window: null pointer");
+    if (k0 < 0 || nk < 1 || k0 + nk > h->nz || ni < 1 || ni > h->Lx)
+        return fail(LBM_ERR_INVALID, "lbm_get_window: rows [%d, %d) of %d, %d columns of %d", k0, k0 + nk, h->nz, ni, h->Lx);
+    dim3 grid((ni + lbm::AUX_TX - 1) / lbm::AUX_TX, nk, LBM_NPOP);
+    lbm::window_kernel<<<grid, lbm::AUX_TX, 0, (cudaStream_t)stream>>>(h->buf[h->cur], h->layout(), k0, nk, i0, ni, f_dev);
     LAUNCHED(h);
     return LBM_OK;
 }
@@ -561,14 +594,30 @@ int lbm_step(lbm_t *h, int n, void *stream)
     if (h->variant == 3 && !plan.fused)
         return fail(LBM_ERR_CUDA, "lbm_step: the two-step kernel needs two lattice copies and tensor maps%s",
                     h->tma_ok ? "" : " (cuTensorMapEncodeTiled failed)");
-    const int launches = plan.fused ? n / 2 + n % 2 : n;
+    const bool persistent = h->persist_blocks > 0 && h->variant == 0 && !plan.fused && n >= 2;
     // Under stream capture the handle's bookkeeping (which copy is current) advances at capture time, not at replay:
-    // a captured sequence must leave the current copy / layout where it was, i.e. hold an even number of launches.
+    // a captured sequence must leave the current copy / layout where it was, i.e. swap the copies an even number of times.
+    const int swaps = persistent ? n : plan.fused ? n / 2 + n % 2 : n;
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
-    if (cap != cudaStreamCaptureStatusNone && launches % 2)
-        return fail(LBM_ERR_INVALID, "lbm_step: %d steps are %d launches here; a captured sequence must hold an even "
-                    "number of launches (the ping-pong must return to the same copy)", n, launches);
+    if (cap != cudaStreamCaptureStatusNone && swaps % 2)
+        return fail(LBM_ERR_INVALID, "lbm_step: %d steps swap the lattice copies %d times here; a captured sequence must "
+                    "swap them an even number of times (the ping-pong must return to the same copy)", n, swaps);
+    if (persistent) {       // small lattice: all n steps in one cooperative launch (lbm_step.cuh)
+        CUDA_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(unsigned), st));
+        double *b0 = h->buf[0], *b1 = h->buf[1];
+        int cur = h->cur, nn = n;
+        void *args[] = {&a, &b0, &b1, &cur, &nn, &h->d_counter};
+        const void *fn = h->persist_tb == 64
+                             ? (h->wall_kind == 1 ? (const void *)lbm::step_persistent_kernel<64, true> : (const void *)lbm::step_persistent_kernel<64, false>)
+                             : (h->wall_kind == 1 ? (const void *)lbm::step_persistent_kernel<128, true> : (const void *)lbm::step_persistent_kernel<128, false>);
+        CUDA_TRY(cudaLaunchCooperativeKernel(fn, dim3(h->persist_blocks), dim3(h->persist_tb), args, 0, st));
+        h->launches++;
+        h->wrap_ok[0] = h->wrap_ok[1] = false;
+        if (n % 2) h->cur ^= 1;
+        h->steps += n;
+        return LBM_OK;
+    }
     int s = 0;
     if (plan.fused && n >= 2) {
         dim3 grid(plan.strips, plan.chunks);

@@ -114,6 +114,22 @@ __global__ void __launch_bounds__(AUX_TX) unpack_kernel(const double *__restrict
     dense[((long long)blockIdx.z * g.nz + j) * g.Lx + i] = *p;
 }
 
+// dense [37][nk][ni] window of the stored state: rows k0 .. k0+nk-1 of the OWN rows, columns i0 .. i0+ni-1 (mod Lx);
+// grid = (ceil(ni/AUX_TX), nk, NPOP)
+__global__ void __launch_bounds__(AUX_TX)
+window_kernel(const double *__restrict__ src, Layout g, int k0, int nk, int i0, int ni, double *dense)
+{
+    const int c = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y, l = blockIdx.z;
+    if (c >= ni) return;
+    int i = (i0 + c) % g.Lx;
+    if (i < 0) i += g.Lx;
+    const double *p = nullptr;
+    each_stored_site(src, g.Lx, g.Lz, g.pitch, g.plane, g.layout_m, i, g.k0 + k0 + j, [&](auto L, const double *q) {
+        if (decltype(L)::value == l) p = q;
+    });
+    dense[((long long)l * nk + j) * ni + c] = *p;
+}
+
 // a1 for the two-step kernel's TMA loads: the XW wrap columns on either side of a row hold the periodic images
 // (column j < 0 holds column j mod Lx, column Lx + j holds column j mod Lx).  The two-step kernel's consumers keep
 // them current themselves; this kernel refreshes them after anything else has written the lattice.

@@ -156,6 +156,46 @@ __global__ void __launch_bounds__(TX *TZ, 512 / (TX * TZ)) step_kernel_site(cons
     scatter_site(a, i, k, f);
 }
 
+// ---- small lattices: n time steps in ONE launch.  A lattice of a few thousand sites is updated in less time than a
+// kernel launch takes (64 x 128: ~1 us of work, ~4 us per launched step), so for lattices that fit one site per
+// resident thread the whole step loop runs inside a persistent cooperative kernel: every thread owns one site, the
+// two copies alternate, and the steps are separated by a grid-wide barrier (one atomic per block on a counter in
+// global memory, polled with acquire loads; the block barrier before it and the fence make the block's stores
+// visible).  Loads bypass L1 (the other copy was rewritten by other SMs a moment ago).  Same gather, same collision:
+// bit-identical to n launches of the one-step kernel.
+template <int TB, bool ISO>
+__global__ void __launch_bounds__(TB) step_persistent_kernel(StepArgs a, double *buf0, double *buf1, int cur, const int nsteps,
+                                                             unsigned *counter)
+{
+    const int site = blockIdx.x * TB + threadIdx.x;
+    const int k = site / a.Lx, i = site - k * a.Lx;
+    const bool live = k < a.Lz;
+    for (int s = 0; s < nsteps; ++s, cur ^= 1) {
+        a.src = cur ? buf1 : buf0;
+        a.dst = cur ? buf0 : buf1;
+        if (live) {
+            double f[NPOP];
+            each_source_site<true>(a, i, k, [&](auto L, const double *p, bool) { f[decltype(L)::value] = __ldcg(p); });
+            wall_rows_adjust<ISO>(a, k, f);
+            d2q37::collide_site(f, a.omega, a.gtau, a.dT);
+            scatter_site(a, i, k, f);
+        }
+        if (s + 1 < nsteps) {                                // grid barrier
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                __threadfence();
+                atomicAdd(counter, 1u);
+                const unsigned target = (unsigned)(s + 1) * gridDim.x;
+                unsigned seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
+                } while (seen < target);
+            }
+            __syncthreads();
+        }
+    }
+}
+
 // ---- in-place streaming: ONE lattice copy ("we keep in memory two copies of the lattice ... This choice
 // requires more memory").  Every site reads 37 slots and writes its 37 results back into the SAME slots, so no slot
 // is touched by two sites in a step and no second copy is needed.  Two alternating kernels:

@@ -3,14 +3,14 @@
 
     python -m paper_1405_1253_b200.run_rt --config 2 [--steps N] [--every 100] [--out widths.csv]
 
-Every `--every` steps it calls lbm_mixing_widths (eq. 12) and lbm_totals and writes
-step, t/tau_RT, L_u, L_d, L_tot, mass, alpha_tot (eq. 14 via lbm_growth_rate), with tau_RT = sqrt(Lx / (g At)) and
-At = (T_d - T_u)/(T_d + T_u) (Table II).  All arithmetic runs in the CUDA library.
+Every `--every` steps it calls lbm_diagnostics (mixing widths of eq. 12, and the lattice totals in
+one pass over the lattice) and writes step, t/tau_RT, L_u, L_d, L_tot, mass, alpha_tot (eq. 14 via lbm_growth_rate),
+with tau_RT = sqrt(Lx / (g At)) and At = (T_d - T_u)/(T_d + T_u) (Table II) from
+lbm_rt_scales.  All arithmetic runs in the library.  --wall-kind 1: isothermal walls at T_d / T_u (reading 19).
 """
 from __future__ import annotations
 
 import argparse
-import math
 import os
 import sys
 import time
@@ -20,22 +20,21 @@ sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 import synthetic_inputs as si  # noqa: E402
 
 
-def run(cfg, steps: int, every: int, seed: int = si.DEFAULT_SEED, out=None, variant: int | None = None):
+def run(cfg, steps: int, every: int, seed: int = si.DEFAULT_SEED, out=None, variant: int | None = None,
+        wall_kind: int = 0, inplace: bool = False):
     import torch
 
     import paper_1405_1253_b200 as pkg
-    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, wall_kind=wall_kind, T_wall=(cfg.T_d, cfg.T_u), inplace=inplace)
     if variant is not None:
         lat.set_variant(variant)
     lat.init_rt(seed, **cfg.rt_args())
-    At = (cfg.T_d - cfg.T_u) / (cfg.T_d + cfg.T_u)
-    tau_rt = math.sqrt(cfg.Lx / (cfg.g * At))
+    At, tau_rt = pkg.rt_scales(cfg.Lx, cfg.g, cfg.T_d, cfg.T_u)
     rows = []
 
     def log():
-        lu, ld, _ = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)
-        mass = lat.totals()[0]
-        rows.append((lat.steps_done, lat.steps_done / tau_rt, lu, ld, lu + ld, mass))
+        d = lat.diagnostics(cfg.T_d, cfg.T_m, cfg.T_u, profiles=False)
+        rows.append((lat.steps_done, lat.steps_done / tau_rt, d["L_u"], d["L_d"], d["L_u"] + d["L_d"], d["totals"][0]))
 
     log()
     torch.cuda.synchronize()
@@ -62,11 +61,13 @@ def main():
     ap.add_argument("--every", type=int, default=100)
     ap.add_argument("--seed", type=int, default=si.DEFAULT_SEED)
     ap.add_argument("--out", default="")
+    ap.add_argument("--wall-kind", type=int, default=0)
+    ap.add_argument("--inplace", action="store_true")
     args = ap.parse_args()
     cfg = si.rt_config(args.config)
     steps = args.steps or cfg.steps
     fh = open(args.out, "w") if args.out else None
-    rows, wall = run(cfg, steps, args.every, args.seed)
+    rows, wall = run(cfg, steps, args.every, args.seed, wall_kind=args.wall_kind, inplace=args.inplace)
     if fh:
         fh.write("step,t_over_tau,L_u,L_d,L_tot,mass,alpha_tot\n")
         for r in rows:

@@ -185,3 +185,38 @@ def test_two_step_kernel_bitwise_at_the_large_lattice_plan(pkg):
         lat.step(50)
     assert torch.equal(a.get_populations(), b.get_populations())
     a.close(); b.close()
+
+
+def test_inplace_16384x16384_one_copy_windows_against_oracle(pkg, orc):
+    """16384 x 16384 (80 GB for ONE lattice copy; two would not leave room for anything else on a 180 GB
+    device) with in-place streaming: equilibrium of the seeded config-5 fields, NSTEPS steps (ending in the shifted
+    layout, NSTEPS is odd), windows through lbm_get_window against the oracle's own equilibrium + steps: walls, seam,
+    bulk, element offsets beyond 2^33."""
+    import torch
+    Lx = Lz = 16384
+    lat = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G, inplace=True)
+    fields = si.sweep_fields_torch(Lx, Lz, si.DEFAULT_SEED, "cuda")
+    lat.init_equilibrium(*fields)
+    del fields
+    torch.cuda.empty_cache()
+    W = 40 + 2 * M
+    cases = [(0, Lx - W // 2 - 1, "bottom"), (Lz - W, Lx // 2 + 5, "top"), (Lz // 2 - 7, 3, "bulk"), (Lz - W - 1000, Lx - W // 2 - 3, "bulk")]
+    before = [lat.get_window(r0, W, c0, W).cpu().numpy() for r0, c0, _ in cases]
+    # the oracle's own equilibrium of the same seeded fields on the first window
+    r0, c0, _ = cases[2]
+    host = si.sweep_fields(Lx, Lz, si.DEFAULT_SEED, rows=slice(r0, r0 + W))
+    ref0 = orc.init_equilibrium(*[np.ascontiguousarray(x[:, c0:c0 + W]) for x in host])
+    assert float(np.max(np.abs(before[2] - ref0) / ref0)) < 1e-13
+    lat.step(NSTEPS)
+    assert NSTEPS % 2 == 1
+    worst = 0.0
+    for (r0, c0, kind), w0 in zip(cases, before):
+        w1 = lat.get_window(r0, W, c0, W).cpu().numpy()
+        ref = orc.step(w0, si.SWEEP_TAU, si.SWEEP_G, nsteps=NSTEPS, periodic_z=(kind == "bulk"))
+        rows = slice(0, W - M) if kind == "bottom" else slice(M, W) if kind == "top" else slice(M, W - M)
+        a, b = w1[:, rows, M:W - M], ref[:, rows, M:W - M]
+        worst = max(worst, float(np.max(np.abs(a - b) / np.abs(b))))
+    assert worst < 1e-13, worst
+    t = lat.totals()
+    assert abs(t[0] / (Lx * Lz) - 1) < 1e-3                   # rho = 1 +- 0.01 per site
+    lat.close()
