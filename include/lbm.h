@@ -6,6 +6,8 @@
  * BGK collision toward the force-shifted equilibrium of eq. 6 with the moments of eq. 7
  * (PAPER.md:88), on an Lx x Lz lattice in FP64, plus the diagnostics of PAPER.md:94, 128 and eq. 12.
  * Every arithmetic step runs in CUDA kernels for sm_100a; there is no CPU fallback.
+ * Beyond the time step: isothermal walls (wall_kind 1), one-copy in-place streaming (pop_buf1 = NULL) and z-slabs
+ * with exchanged ghost rows (lbm_create_slab) -- SURVEY.md 8(f) rows 2-4.
  *
  * Conventions.  Sites (i,k): i = 0..Lx-1 along x (periodic), k = 0..Lz-1 along z (up, walls half a site
  * outside rows 0 and Lz-1).  Canonical dense arrays are x-fastest: fields [Lz][Lx], populations
@@ -199,9 +201,11 @@ int lbm_kernel_launches(const lbm_t *h, long long *launches);       /* kernels l
  * events on `stream` and returns the vector-FP64 rate in TFLOP/s (FMA = 2 flops) in HOST *tflops.  Not part of the
  * time step.  Synchronises `stream`. */
 int lbm_fp64_peak(double *tflops, int iters, void *stream);
-/* Step-kernel variant: 0 automatic (default), 1 one step per launch (256-thread blocks), 2 one step (128),
- * 3 two steps per launch forced (lbm_step2s.cuh; automatic picks it from about 512x1024 up).  All give
- * bit-identical results. */
+/* Step-kernel variant: 0 automatic (default): the two-step kernel (lbm_step2s.cuh) where its launch plan is
+ * predicted faster than two single steps (from about 512x512 up), one cooperative launch for all n steps on
+ * lattices of at most ~37 000 sites (persistent kernel with a grid barrier between steps), else one step per
+ * launch; 1 one step per launch (256-thread blocks), 2 one step (128), 3 two steps per launch forced
+ * (LBM_ERR_CUDA from lbm_step for in-place handles: it needs two copies).  All give bit-identical results. */
 int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel (>= 3), or 0 = automatic */
 /* The launch plan lbm_step uses for this lattice with the current variant / zchunk settings (HOST outputs, any may
