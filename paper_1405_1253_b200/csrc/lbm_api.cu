@@ -224,10 +224,11 @@ const lbm_plan &make_plan(lbm_t *h)
         p.chunks = (Lz + p.ZC - 1) / p.ZC;
         best = ((double)(((long long)p.strips * p.chunks + sms - 1) / sms) + 0.3) * (p.ZC + 10);
     }
-    // predicted time of two steps, microseconds: the two-step kernel spends ~0.85 us per row of a chunk (1.7 us per
-    // pass of two rows) plus ~4 us per launch; the one-step kernel ~92 ps per site and step plus ~3 us per launch
+    // predicted time of two steps, microseconds: the two-step kernel spends ~0.65-0.7 us per unit of the cost above
+    // on lattices of up to a few million sites (1.3-1.4 us per pass of two rows; the largest lattices, DRAM- and
+    // power-bound, need 0.9) plus ~4 us per launch; the one-step kernel ~92 ps per site and step plus ~3 us per launch
     // (profiles/r2_sweep.md)
-    const double t_fused = 0.85 * best + 4.0;
+    const double t_fused = 0.70 * best + 4.0;
     const double t_single = 2.0 * (92e-6 * (double)Lx * Lz + 3.0);
     const bool can_fuse = h->tma_ok && !h->inplace && !h->slab;
     p.fused = can_fuse && (h->variant == 3 || (h->variant == 0 && t_fused < t_single));

@@ -246,3 +246,41 @@ def test_graph_capture_of_the_two_step_kernel_and_odd_launch_counts(pkg):
     torch.cuda.synchronize()
     assert torch.equal(a.get_populations(), b.get_populations())
     a.close(); b.close()
+
+
+def test_two_step_kernel_soak_on_an_l2_resident_lattice(pkg):
+    """the stage hand-off (generic-proxy reads, then the TMA unit rewrites the buffer) is most exposed when
+    the source rows come from L2 and the boxes land fast: 256x512 (both copies L2-resident), two-step kernel forced,
+    3000 steps in batches, compared bit for bit with the one-step kernel after every batch."""
+    import torch
+    Lx, Lz = 256, 512
+    fields = si.sweep_fields_torch(Lx, Lz, 9, "cuda")
+    a, b = pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G), pkg.Lattice(Lx, Lz, si.SWEEP_TAU, si.SWEEP_G)
+    a.set_variant(1); b.set_variant(3)
+    assert b.plan()[0]
+    for lat in (a, b):
+        lat.init_equilibrium(*fields)
+    for _ in range(6):
+        a.step(500); b.step(500)
+        assert torch.equal(a.get_populations(), b.get_populations())
+    a.close(); b.close()
+
+
+def test_a_handle_rejects_calls_from_another_device(pkg):
+    """a handle belongs to the device that was current in lbm_create (the shared-memory opt-in, the tensor
+    maps and the scratch live there); with another device current every device call is refused.  Needs two GPUs."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    lat0 = pkg.Lattice(512, 1024, 0.8, 1e-4, device="cuda:0")
+    lat1 = pkg.Lattice(512, 1024, 0.8, 1e-4, device="cuda:1")
+    cfg = si.rt_config(2)
+    for lat in (lat0, lat1):
+        lat.init_rt(1, **cfg.rt_args())
+        lat.step(4)                                           # the fused path on both devices
+    assert torch.equal(lat0.get_populations().cpu(), lat1.get_populations().cpu())
+    import ctypes as C
+    with torch.cuda.device(0):                                # the raw call, bypassing the binding's device guard
+        rc = lat1._lib.lbm_step(lat1._h, 2, C.c_void_p(0))
+    assert rc == -1
+    lat0.close(); lat1.close()
