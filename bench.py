@@ -423,6 +423,71 @@ def run_slabs(args):
     dist.destroy_process_group()
 
 
+def run_slabs_local(args):
+    """--slabs-local K: the N = 1 workload cut into K z-slabs that all live on THIS device, ghost rows exchanged every
+    step by device-to-device copies on a second stream while the interior rows run (the machinery of --slabs without the
+    network): measures what packing, unpacking and the interior/edge split cost against the whole lattice stepped with
+    the same one-step kernel.  Prints one JSON line; not the driver's contract line."""
+    import torch
+
+    import __graft_entry__ as entry
+    import paper_1405_1253_b200 as pkg
+    from paper_1405_1253_b200.slab_ring import partition
+    entry.build()
+    torch.cuda.set_device(0)
+    cfg = si.rt_config(args.config)
+    if args.lx and args.lz:
+        cfg = si.scaled(cfg, args.lx, args.lz)
+    main = torch.cuda.current_stream()
+    xs = torch.cuda.Stream()
+    K = args.slabs_local
+
+    def timed(fn):
+        fn(args.warmup)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(main); fn(args.steps); e1.record(main)
+        torch.cuda.synchronize()
+        return cfg.Lx * cfg.Lz * args.steps / (e0.elapsed_time(e1) * 1e-3) / 1e6
+
+    whole = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    whole.set_variant(1)
+    whole.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    mlups_whole = timed(whole.step)
+    whole.close()
+    del whole
+    torch.cuda.empty_cache()
+    slabs = [pkg.Slab(cfg.Lx, cfg.Lz, z0, nz, cfg.tau, cfg.g) for z0, nz in partition(cfg.Lz, K)]
+    for s in slabs:
+        s.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    up, dn, below, above = ([s.new_message() for s in slabs] for _ in range(4))
+
+    def step_slabs(n):
+        for _ in range(n):
+            xs.wait_stream(main)
+            with torch.cuda.stream(xs):
+                for i, s in enumerate(slabs):
+                    if s.open_above: s.pack(1, up[i], stream=xs)
+                    if s.open_below: s.pack(0, dn[i], stream=xs)
+            for s in slabs:
+                s.step_part(s.INTERIOR, stream=main)
+            with torch.cuda.stream(xs):
+                for i, s in enumerate(slabs):
+                    if s.open_below: below[i].copy_(up[i - 1], non_blocking=True); s.unpack(0, below[i], stream=xs)
+                    if s.open_above: above[i].copy_(dn[i + 1], non_blocking=True); s.unpack(1, above[i], stream=xs)
+            main.wait_stream(xs)
+            for s in slabs:
+                s.step_part(s.EDGES, stream=main)
+
+    mlups_slabs = timed(step_slabs)
+    print(json.dumps({"slabs_local": K, "workload": cfg.name, "Lx": cfg.Lx, "Lz": cfg.Lz, "steps": args.steps,
+                      "mlups_whole_lattice_one_step_kernel": mlups_whole, "mlups_slabs": mlups_slabs,
+                      "ratio": mlups_slabs / mlups_whole, "message_bytes": 26 * cfg.Lx * 8,
+                      "launches_per_step": sum(2 * (s.open_above + s.open_below) + 1 + (s.open_above + s.open_below) for s in slabs)}))
+    for s in slabs:
+        s.close()
+
+
 def run_sweep(args):
     """--sweep: BASELINE.json configs[4] -- steady-state throughput from 256x512 to 8192x16384, populations at
     the equilibrium of i.i.d. rho, T, u fields; 200 timed steps per size (after 10 warm-up), one JSON line per
@@ -486,6 +551,7 @@ def main():
     ap.add_argument("--sweep-variants", default="0")
     ap.add_argument("--inplace", action="store_true", help="sweep with ONE lattice copy (in-place streaming)")
     ap.add_argument("--slabs", action="store_true", help="N > 1: one lattice cut into z-slabs over the ranks (strong scaling)")
+    ap.add_argument("--slabs-local", type=int, default=0, help="K z-slabs on this one device (cost of the slab machinery)")
     ap.add_argument("--sweep-sizes", default="", help="e.g. 256x512,4096x8192 (default: all of config 5)")
     args = ap.parse_args()
     if args.warmup < 3:
@@ -494,6 +560,8 @@ def main():
         run_sweep(args)
     elif args.slabs:
         run_slabs(args)
+    elif args.slabs_local:
+        run_slabs_local(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

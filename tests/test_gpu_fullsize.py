@@ -220,3 +220,25 @@ def test_inplace_16384x16384_one_copy_windows_against_oracle(pkg, orc):
     t = lat.totals()
     assert abs(t[0] / (Lx * Lz) - 1) < 1e-3                   # rho = 1 +- 0.01 per site
     lat.close()
+
+
+def test_two_slabs_of_config3_equal_the_whole_lattice_after_100_steps(pkg):
+    """SURVEY 8(f)4 on one device: the 2048x4096 lattice of config 3 as two z-slabs, ghost rows exchanged every step by
+    device-to-device copies on a second stream while the interior rows run, against the whole lattice stepped with the
+    default plan (two-step kernel): bit-identical after 100 steps."""
+    import torch
+    from test_gpu_variants import _run_slabs
+    cfg = si.rt_config(3)
+    whole = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    assert whole.plan()[0]
+    whole.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    whole.step(100)
+    ref = whole.get_populations()
+    whole.close()
+    slabs = [pkg.Slab(cfg.Lx, cfg.Lz, z0, nz, cfg.tau, cfg.g) for z0, nz in ((0, 2048), (2048, 2048))]
+    for s in slabs:
+        s.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    _run_slabs(pkg, slabs, 100)
+    for s, rows in zip(slabs, (slice(0, 2048), slice(2048, 4096))):
+        assert torch.equal(s.get_populations(), ref[:, rows])
+        s.close()

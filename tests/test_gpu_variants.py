@@ -129,16 +129,20 @@ def _run_slabs(pkg, slabs, nsteps, exchange_stream=None):
     xs = exchange_stream or torch.cuda.Stream()
     up = [s.new_message() for s in slabs]      # message of slab i to the slab above
     dn = [s.new_message() for s in slabs]
+    from_below = [s.new_message() for s in slabs]   # receive buffers
+    from_above = [s.new_message() for s in slabs]
     for _ in range(nsteps):
         xs.wait_stream(main)
-        for i, s in enumerate(slabs):
-            if s.open_above: s.pack(1, up[i], stream=xs)
-            if s.open_below: s.pack(0, dn[i], stream=xs)
+        with torch.cuda.stream(xs):
+            for i, s in enumerate(slabs):
+                if s.open_above: s.pack(1, up[i], stream=xs)
+                if s.open_below: s.pack(0, dn[i], stream=xs)
         for s in slabs:
             s.step_part(pkg.Slab.INTERIOR, stream=main)
-        for i, s in enumerate(slabs):                         # "transport": the neighbour's message, same device here
-            if s.open_below: s.unpack(0, up[i - 1], stream=xs)
-            if s.open_above: s.unpack(1, dn[i + 1], stream=xs)
+        with torch.cuda.stream(xs):
+            for i, s in enumerate(slabs):                     # "transport": device-to-device copies (cudaMemcpyAsync)
+                if s.open_below: from_below[i].copy_(up[i - 1], non_blocking=True); s.unpack(0, from_below[i], stream=xs)
+                if s.open_above: from_above[i].copy_(dn[i + 1], non_blocking=True); s.unpack(1, from_above[i], stream=xs)
         main.wait_stream(xs)
         for s in slabs:
             s.step_part(pkg.Slab.EDGES, stream=main)
