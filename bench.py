@@ -480,8 +480,32 @@ def run_slabs_local(args):
                 s.step_part(s.EDGES, stream=main)
 
     mlups_slabs = timed(step_slabs)
+
+    # the same slabs with the two-step kernel: 6 whole ghost rows per open side and pair of steps, no interior/edge split
+    up2, dn2, below2, above2 = ([s.new_message(True) for s in slabs] for _ in range(4))
+
+    def step_slabs_fused(n):
+        for _ in range(n // 2):
+            for i, s in enumerate(slabs):
+                if s.open_above: s.pack2(1, up2[i])
+                if s.open_below: s.pack2(0, dn2[i])
+            for i, s in enumerate(slabs):
+                if s.open_below: below2[i].copy_(up2[i - 1], non_blocking=True); s.unpack2(0, below2[i])
+                if s.open_above: above2[i].copy_(dn2[i + 1], non_blocking=True); s.unpack2(1, above2[i])
+            for s in slabs:
+                s.step2()
+
+    mlups_fused = timed(step_slabs_fused)
+    mlups_whole2 = None
+    if torch.cuda.mem_get_info()[0] > 2.2 * pkg.buffer_bytes(cfg.Lx, cfg.Lz):      # room for the whole lattice beside the slabs
+        whole2 = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+        whole2.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+        mlups_whole2 = timed(whole2.step)
+        whole2.close()
     print(json.dumps({"slabs_local": K, "workload": cfg.name, "Lx": cfg.Lx, "Lz": cfg.Lz, "steps": args.steps,
                       "mlups_whole_lattice_one_step_kernel": mlups_whole, "mlups_slabs": mlups_slabs,
+                      "mlups_whole_lattice_default_plan": mlups_whole2, "mlups_slabs_two_step_kernel": mlups_fused,
+                      "message2_bytes": 6 * 37 * (cfg.Lx + 16) * 8,
                       "ratio": mlups_slabs / mlups_whole, "message_bytes": 26 * cfg.Lx * 8,
                       "launches_per_step": sum(2 * (s.open_above + s.open_below) + 1 + (s.open_above + s.open_below) for s in slabs)}))
     for s in slabs:

@@ -91,7 +91,8 @@ int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p);
 /* ---- z-slabs: the lattice split along z over several handles (one per GPU), SURVEY 8(f)4.  The paper splits
  * along x over N_p GPUs and hides the halo exchange behind the bulk propagate on separate streams (PAPER.md:110,
  * 116-118, Fig. 3-4); with x-fastest storage the contiguous cut is along z.
- * A slab owns rows [z0, z0+nz) of an Lx x Lz_global lattice and stores 3 ghost rows per open side (max |e_z| = 3).
+ * A slab owns rows [z0, z0+nz) of an Lx x Lz_global lattice and stores 6 ghost rows per open side (one step reads 3,
+ * max |e_z| = 3; two fused steps read 6).
  * Dense arrays of every other call (fields [nz][Lx], populations [37][nz][Lx], row profiles [nz]) cover the OWN rows;
  * lbm_totals and the widths of lbm_mixing_widths are the slab's partial sums (add them over the slabs).
  * One time step of a slab, every step:
@@ -100,20 +101,31 @@ int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p);
  *   ... the caller moves the messages (cudaMemcpyAsync between devices, ncclSend/ncclRecv, ...) ...
  *   lbm_slab_unpack(side)    neighbour's message -> my ghost rows of the CURRENT copy
  *   lbm_slab_step(EDGES)     the remaining own rows; then the other copy becomes current.
- * Results are bit-identical to the whole-lattice run.  Slabs use the one-step kernel and two lattice copies;
+ * Two steps at once with the two-step kernel (lbm_step2s.cuh), no interior/edge split -- the exchange is a few
+ * microseconds beside milliseconds of stepping:
+ *   lbm_slab_pack2(side)     my 6 outermost own rows, all populations, wrap columns included -> message
+ *   ... transport ...
+ *   lbm_slab_unpack2(side)   neighbour's message -> my 6 ghost rows of the CURRENT copy
+ *   lbm_slab_step2           two time steps of the own rows; then the other copy becomes current.
+ * Results are bit-identical to the whole-lattice run.  Slabs need two lattice copies;
  * lbm_step / lbm_run_host return LBM_ERR_INVALID for them.  lbm_init_rt fills ghost rows too (closed form);
  * after lbm_init_equilibrium / lbm_set_populations the first exchange does. */
 #define LBM_SLAB_INTERIOR 0
 #define LBM_SLAB_EDGES 1
 size_t lbm_slab_buffer_bytes(int Lx, int Lz_global, int z0, int nz);   /* 0 if invalid (nz >= 6 rows inside the lattice) */
 int lbm_create_slab(lbm_t **out, int Lx, int Lz_global, int z0, int nz, const lbm_params *p);
-/* HOST outputs, any may be NULL: own row range, whether the sides are open (1) or walls (0), doubles per message. */
-int lbm_slab_info(const lbm_t *h, int *z0, int *nz, int *open_below, int *open_above, size_t *message_doubles);
+/* HOST outputs, any may be NULL: own row range, whether the sides are open (1) or walls (0), doubles per message of
+ * lbm_slab_pack (26 Lx) and of lbm_slab_pack2 (6 x 37 x (Lx + 16)). */
+int lbm_slab_info(const lbm_t *h, int *z0, int *nz, int *open_below, int *open_above, size_t *message_doubles,
+                  size_t *message2_doubles);
 /* side 0 = towards lower z, 1 = towards higher z; msg_dev: DEVICE buffer of message_doubles doubles; asynchronous.
  * LBM_ERR_INVALID if that side is a wall. */
 int lbm_slab_pack(lbm_t *h, int side, double *msg_dev, void *stream);
 int lbm_slab_unpack(lbm_t *h, int side, const double *msg_dev, void *stream);
 int lbm_slab_step(lbm_t *h, int part, void *stream);
+int lbm_slab_pack2(lbm_t *h, int side, double *msg_dev, void *stream);
+int lbm_slab_unpack2(lbm_t *h, int side, const double *msg_dev, void *stream);
+int lbm_slab_step2(lbm_t *h, void *stream);
 
 /* Frees the handle and its scratch; never the population buffers. NULL is a no-op. */
 int lbm_destroy(lbm_t *h);

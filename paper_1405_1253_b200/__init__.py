@@ -282,13 +282,30 @@ class Slab(Lattice):
                  T_wall=(1.0, 1.0), device="cuda"):
         super().__init__(Lx, nz, tau, g, wall_kind=wall_kind, T_wall=T_wall, device=device, _slab=(Lz_global, z0, nz))
         self.Lz_global, self.z0, self.nz = int(Lz_global), int(z0), int(nz)
-        z, n, lo, hi, m = C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_size_t()
-        binding.check(self._lib.lbm_slab_info(self._h, C.byref(z), C.byref(n), C.byref(lo), C.byref(hi), C.byref(m)))
-        self.open_below, self.open_above, self.message_doubles = bool(lo.value), bool(hi.value), int(m.value)
+        z, n, lo, hi, m, m2 = C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_size_t(), C.c_size_t()
+        binding.check(self._lib.lbm_slab_info(self._h, C.byref(z), C.byref(n), C.byref(lo), C.byref(hi), C.byref(m),
+                                              C.byref(m2)))
+        self.open_below, self.open_above = bool(lo.value), bool(hi.value)
+        self.message_doubles, self.message2_doubles = int(m.value), int(m2.value)
 
-    def new_message(self):
+    def new_message(self, two_steps: bool = False):
+        """A device buffer for one message of pack / unpack (two_steps: of pack2 / unpack2)."""
         import torch
-        return torch.empty(self.message_doubles, dtype=torch.float64, device=self.device)
+        return torch.empty(self.message2_doubles if two_steps else self.message_doubles, dtype=torch.float64,
+                           device=self.device)
+
+    @_on_device
+    def pack2(self, side: int, msg, stream=None):
+        binding.check(self._lib.lbm_slab_pack2(self._h, int(side), _dptr(msg), _stream_ptr(stream, self.device)))
+
+    @_on_device
+    def unpack2(self, side: int, msg, stream=None):
+        binding.check(self._lib.lbm_slab_unpack2(self._h, int(side), _dptr(msg), _stream_ptr(stream, self.device)))
+
+    @_on_device
+    def step2(self, stream=None):
+        """Two time steps of the slab's own rows with the two-step kernel (after pack2 / transport / unpack2)."""
+        binding.check(self._lib.lbm_slab_step2(self._h, _stream_ptr(stream, self.device)))
 
     @_on_device
     def pack(self, side: int, msg, stream=None):

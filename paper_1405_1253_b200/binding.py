@@ -20,7 +20,7 @@ SYMBOLS = [
     "lbm_step", "lbm_moments", "lbm_mixing_widths", "lbm_profiles", "lbm_growth_rate", "lbm_totals", "lbm_run_host", "lbm_steps_done",
     "lbm_layout", "lbm_kernel_launches", "lbm_fp64_peak", "lbm_set_variant", "lbm_set_zchunk", "lbm_get_plan", "lbm_tables", "lbm_last_error",
     "lbm_diagnostics", "lbm_rt_scales", "lbm_slab_buffer_bytes", "lbm_create_slab", "lbm_slab_info", "lbm_slab_pack",
-    "lbm_slab_unpack", "lbm_slab_step", "lbm_get_window",
+    "lbm_slab_unpack", "lbm_slab_step", "lbm_get_window", "lbm_slab_pack2", "lbm_slab_unpack2", "lbm_slab_step2",
 ]
 
 
@@ -83,7 +83,10 @@ def load():
     L.lbm_slab_buffer_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int]
     L.lbm_create_slab.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(lbm_params)]
     L.lbm_slab_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int),
-                                C.POINTER(C.c_size_t)]
+                                C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+    L.lbm_slab_pack2.argtypes = [vp, C.c_int, vp, vp]
+    L.lbm_slab_unpack2.argtypes = [vp, C.c_int, vp, vp]
+    L.lbm_slab_step2.argtypes = [vp, vp]
     L.lbm_slab_pack.argtypes = [vp, C.c_int, vp, vp]
     L.lbm_slab_unpack.argtypes = [vp, C.c_int, vp, vp]
     L.lbm_slab_step.argtypes = [vp, C.c_int, vp]

@@ -37,7 +37,8 @@ int fail(int code, const char *fmt, ...)
 
 constexpr int ROW_ALIGN = 16;     // doubles: rows start on 128-byte lines
 constexpr int PLANE_PAD = 272;    // doubles (17 x 128 B): keeps the 37 plane bases off a power-of-two stride
-constexpr int GHOST = 3;          // ghost rows per open side of a z-slab (max |e_z|)
+constexpr int GHOST = 3;          // ghost rows one step reads beyond an open side of a z-slab (max |e_z|)
+constexpr int GHOST_STORED = 6;   // ghost rows stored per open side: two fused steps read 6
 
 // row = [XH spare | Lx sites | XH spare], padded to 128 bytes
 int pitch_of(int Lx) { return (Lx + 2 * lbm::XH + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN; }
@@ -183,6 +184,7 @@ lbm::StepArgs step_args(const lbm_t *h)
     a.Tw_hi = h->T_wall_hi - 0.125 * h->g * h->g;
     a.wrap_store = 0;
     a.w = 0;
+    a.zbase = h->glo; a.zend = h->glo + h->nz;
     lbm::fill_offsets(a);
     return a;
 }
@@ -200,7 +202,7 @@ const lbm_plan &make_plan(lbm_t *h)
     if (h->plan.valid) return h->plan;
     lbm_plan &p = h->plan;
     p = lbm_plan{};
-    const int Lx = h->Lx, Lz = h->Lz, sms = h->sm_count > 0 ? h->sm_count : 148;
+    const int Lx = h->Lx, Lz = h->nz, sms = h->sm_count > 0 ? h->sm_count : 148;   // rows to update: a slab's own
     const int ns_min = (Lx + S2::TX - 1) / S2::TX;
     double best = 1e300;
     for (int ns = ns_min; ns <= ns_min + ns_min / 4 + 1; ++ns) {
@@ -230,7 +232,7 @@ const lbm_plan &make_plan(lbm_t *h)
     // (profiles/r2_sweep.md)
     const double t_fused = 0.70 * best + 4.0;
     const double t_single = 2.0 * (92e-6 * (double)Lx * Lz + 3.0);
-    const bool can_fuse = h->tma_ok && !h->inplace && !h->slab;
+    const bool can_fuse = h->tma_ok && !h->inplace;
     p.fused = can_fuse && (h->variant == 3 || (h->variant == 0 && t_fused < t_single));
     p.valid = true;
     return p;
@@ -284,6 +286,32 @@ void advance(lbm_t *h, int nsteps)
     h->steps += nsteps;
 }
 
+// one launch of the two-step kernel over the rows [zbase, zend) of `a` (lbm_step; lbm_slab_step2)
+int launch_two_step(lbm_t *h, lbm::StepArgs &a, const lbm_plan &plan, cudaStream_t st)
+{
+    using S2 = lbm::Step2sWide;
+    dim3 grid(plan.strips, plan.chunks);
+    a.w = plan.w;
+    // the consumers' spare lanes of the two seam strips keep the wrap columns of the destination current, if the
+    // seam columns [0, XW) and [Lx - XW, Lx) each lie within one strip and that strip has XW lanes to spare (2 XW
+    // if it is the only strip); else the columns are refreshed before every launch
+    const int last = h->Lx - (plan.strips - 1) * plan.w;      // columns of the last strip
+    a.wrap_store = h->Lx >= 2 * lbm::XW && last >= lbm::XW &&
+                   (plan.strips > 1 ? plan.w + lbm::XW <= S2::CW : last + 2 * lbm::XW <= S2::CW);
+    int rc = refresh_wrap_columns(h, h->cur, st);
+    if (rc) return rc;
+    a.src = h->buf[h->cur];
+    a.dst = h->buf[h->cur ^ 1];
+    if (h->wall_kind == 1)
+        lbm::step2s_kernel<S2, true><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], plan.ZC);
+    else
+        lbm::step2s_kernel<S2, false><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], plan.ZC);
+    LAUNCHED(h);
+    h->wrap_ok[h->cur ^ 1] = a.wrap_store != 0;   // the spare lanes of the seam strips wrote the images (own rows)
+    advance(h, 2);                               // a5: swap prv / nxt, once per two steps
+    return LBM_OK;
+}
+
 int create_common(lbm_t **out, int Lx, int rows_stored, const lbm_params *p, const char *fn)
 {
     if (!out) return fail(LBM_ERR_INVALID, "%s: out is null", fn);
@@ -335,7 +363,7 @@ int create_common(lbm_t **out, int Lx, int rows_stored, const lbm_params *p, con
 int finish_create(lbm_t **out)
 {
     lbm_handle *h = *out;
-    if (!h->inplace && !h->slab) {
+    if (!h->inplace) {
         h->tma_ok = encode_step2s_maps(h->ubuf[0], h->Lx, h->Lz, h->pitch, h->plane, h->maps[0]) &&
                     encode_step2s_maps(h->ubuf[1], h->Lx, h->Lz, h->pitch, h->plane, h->maps[1]);
         // the opt-in to > 48 KB of dynamic shared memory is per device (context), so it is made for every handle
@@ -408,7 +436,7 @@ size_t lbm_buffer_bytes(int Lx, int Lz)
 size_t lbm_slab_buffer_bytes(int Lx, int Lz_global, int z0, int nz)
 {
     if (Lx < 7 || Lz_global < 6 || z0 < 0 || nz < GHOST || z0 + nz > Lz_global) return 0;
-    const int rows = nz + (z0 > 0 ? GHOST : 0) + (z0 + nz < Lz_global ? GHOST : 0);
+    const int rows = nz + (z0 > 0 ? GHOST_STORED : 0) + (z0 + nz < Lz_global ? GHOST_STORED : 0);
     return rows < 6 ? 0 : (size_t)plane_of(Lx, rows) * LBM_NPOP * sizeof(double);
 }
 
@@ -437,7 +465,7 @@ int lbm_create_slab(lbm_t **out, int Lx, int Lz_global, int z0, int nz, const lb
         return fail(LBM_ERR_INVALID, "lbm_create_slab: rows [%d, %d) of %d: a slab needs >= %d rows inside the lattice",
                     z0, z0 + nz, Lz_global, 2 * GHOST);
     if (p && !p->pop_buf1) return fail(LBM_ERR_INVALID, "lbm_create_slab: a slab needs two lattice copies");
-    const int glo = z0 > 0 ? GHOST : 0, ghi = z0 + nz < Lz_global ? GHOST : 0;
+    const int glo = z0 > 0 ? GHOST_STORED : 0, ghi = z0 + nz < Lz_global ? GHOST_STORED : 0;
     int rc = create_common(out, Lx, glo + nz + ghi, p, "lbm_create_slab");
     if (rc) return rc;
     lbm_handle *h = *out;
@@ -621,28 +649,9 @@ int lbm_step(lbm_t *h, int n, void *stream)
     }
     int s = 0;
     if (plan.fused && n >= 2) {
-        dim3 grid(plan.strips, plan.chunks);
-        a.w = plan.w;
-        // the consumers' spare lanes of the two seam strips keep the wrap columns of the destination current, if the
-        // seam columns [0, XW) and [Lx - XW, Lx) each lie within one strip and that strip has XW lanes to spare (2 XW
-        // if it is the only strip); else the columns are refreshed before every launch
-        {
-            const int last = h->Lx - (plan.strips - 1) * plan.w;      // columns of the last strip
-            a.wrap_store = h->Lx >= 2 * lbm::XW && last >= lbm::XW &&
-                           (plan.strips > 1 ? plan.w + lbm::XW <= S2::CW : last + 2 * lbm::XW <= S2::CW);
-        }
         for (; s + 2 <= n; s += 2) {
-            int rc = refresh_wrap_columns(h, h->cur, st);
+            int rc = launch_two_step(h, a, plan, st);
             if (rc) return rc;
-            a.src = h->buf[h->cur];
-            a.dst = h->buf[h->cur ^ 1];
-            if (h->wall_kind == 1)
-                lbm::step2s_kernel<S2, true><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], plan.ZC);
-            else
-                lbm::step2s_kernel<S2, false><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], plan.ZC);
-            LAUNCHED(h);
-            h->wrap_ok[h->cur ^ 1] = a.wrap_store != 0;   // the consumers of the seam strips wrote the images
-            advance(h, 2);                               // a5: swap prv / nxt, once per two steps
         }
     }
     for (; s < n; ++s) {
@@ -665,7 +674,8 @@ int lbm_get_plan(lbm_t *h, int *fused, int *strip_width, int *zchunk)
 }
 
 // ---- z-slabs (Fig. 3-4) -------------------------------------------------------
-int lbm_slab_info(const lbm_t *h, int *z0, int *nz, int *open_below, int *open_above, size_t *message_doubles)
+int lbm_slab_info(const lbm_t *h, int *z0, int *nz, int *open_below, int *open_above, size_t *message_doubles,
+                  size_t *message2_doubles)
 {
     NEED_HOST(h);
     if (!h->slab) return fail(LBM_ERR_INVALID, "lbm_slab_info: not a slab handle");
@@ -674,6 +684,7 @@ int lbm_slab_info(const lbm_t *h, int *z0, int *nz, int *open_below, int *open_a
     if (open_below) *open_below = h->glo > 0;
     if (open_above) *open_above = h->ghi > 0;
     if (message_doubles) *message_doubles = (size_t)26 * h->Lx;
+    if (message2_doubles) *message2_doubles = (size_t)GHOST_STORED * LBM_NPOP * (h->Lx + 2 * lbm::XW);
     return LBM_OK;
 }
 
@@ -725,6 +736,49 @@ int lbm_slab_step(lbm_t *h, int part, void *stream)
         return LBM_OK;
     }
     return fail(LBM_ERR_INVALID, "lbm_slab_step: part must be LBM_SLAB_INTERIOR or LBM_SLAB_EDGES (got %d)", part);
+}
+
+// Two fused steps of a slab.  They read 6 ghost rows per open side, complete (all populations) and with their wrap
+// columns: lbm_slab_pack2 / lbm_slab_unpack2 move whole rows.
+int lbm_slab_pack2(lbm_t *h, int side, double *msg_dev, void *stream)
+{
+    NEED(h);
+    if (!h->slab || (side != 0 && side != 1) || !msg_dev) return fail(LBM_ERR_INVALID, "lbm_slab_pack2: slab handle, side 0/1 and a buffer are required");
+    if (side == 0 ? h->glo == 0 : h->ghi == 0) return fail(LBM_ERR_INVALID, "lbm_slab_pack2: side %d of this slab is a wall", side);
+    if (h->slab_phase != 0) return fail(LBM_ERR_INVALID, "lbm_slab_pack2: a one-step slab step is half done");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = refresh_wrap_columns(h, h->cur, st);          // the message carries the images of my rows
+    if (rc) return rc;
+    const int row0 = side == 1 ? h->glo + h->nz - GHOST_STORED : h->glo;
+    dim3 grid((h->Lx + 2 * lbm::XW + lbm::AUX_TX - 1) / lbm::AUX_TX, GHOST_STORED, LBM_NPOP);
+    lbm::slab_rows_kernel<lbm::XW, true><<<grid, lbm::AUX_TX, 0, st>>>(h->buf[h->cur], h->layout(), row0, msg_dev);
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
+int lbm_slab_unpack2(lbm_t *h, int side, const double *msg_dev, void *stream)
+{
+    NEED(h);
+    if (!h->slab || (side != 0 && side != 1) || !msg_dev) return fail(LBM_ERR_INVALID, "lbm_slab_unpack2: slab handle, side 0/1 and a buffer are required");
+    if (side == 0 ? h->glo == 0 : h->ghi == 0) return fail(LBM_ERR_INVALID, "lbm_slab_unpack2: side %d of this slab is a wall", side);
+    const int row0 = side == 1 ? h->glo + h->nz : 0;
+    dim3 grid((h->Lx + 2 * lbm::XW + lbm::AUX_TX - 1) / lbm::AUX_TX, GHOST_STORED, LBM_NPOP);
+    lbm::slab_rows_kernel<lbm::XW, false><<<grid, lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
+        h->buf[h->cur], h->layout(), row0, const_cast<double *>(msg_dev));
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
+int lbm_slab_step2(lbm_t *h, void *stream)
+{
+    NEED(h);
+    if (!h->slab) return fail(LBM_ERR_INVALID, "lbm_slab_step2: not a slab handle");
+    if (h->slab_phase != 0) return fail(LBM_ERR_INVALID, "lbm_slab_step2: a one-step slab step is half done");
+    if (h->nz < GHOST_STORED) return fail(LBM_ERR_INVALID, "lbm_slab_step2: a slab needs at least %d rows", GHOST_STORED);
+    if (!h->tma_ok) return fail(LBM_ERR_CUDA, "lbm_slab_step2: the two-step kernel needs tensor maps (cuTensorMapEncodeTiled failed)");
+    const lbm_plan &plan = make_plan(h);                     // strips and chunks over the slab's own rows
+    lbm::StepArgs a = step_args(h);
+    return launch_two_step(h, a, plan, (cudaStream_t)stream);
 }
 
 // ---- diagnostics (a6) ------------------------------------------------------------------------------------------------

@@ -165,6 +165,21 @@ __global__ void __launch_bounds__(AUX_TX) slab_unpack_kernel(double *dst, Layout
     dst[(long long)sel.l[j] * g.plane + (long long)sel.row[j] * g.pitch + i] = msg[(long long)j * g.Lx + i];
 }
 
+// z-slab messages of the two-step path: whole rows, all 37 populations, wrap columns included (the receiver's TMA
+// boxes read them), `nrows` consecutive stored rows from `row0`.  msg = [nrows][NPOP][Lx + 2 XW].
+// grid = (ceil((Lx + 2 XW)/AUX_TX), nrows, NPOP)
+template <int XW, bool PACK>
+__global__ void __launch_bounds__(AUX_TX) slab_rows_kernel(double *buf, Layout g, int row0, double *msg)
+{
+    const int c = blockIdx.x * AUX_TX + threadIdx.x, j = blockIdx.y, l = blockIdx.z;
+    const int wcols = g.Lx + 2 * XW;
+    if (c >= wcols) return;
+    double *p = buf + (long long)l * g.plane + (long long)(row0 + j) * g.pitch + (c - XW);
+    double *m = msg + ((long long)j * NPOP + l) * wcols + c;
+    if (PACK) *m = *p;
+    else *p = *m;
+}
+
 // Hydrodynamic fields of the stored (post-collision) state: rho, u^(H) = u - g_vec dt/2 = (u_x, u_z + g/2),
 // T^(H) = T + g^2/8 (PAPER.md:94 applied after the collision's u -> u + g_vec dt; reading 8).  grid.y = nz
 __global__ void __launch_bounds__(AUX_TX)

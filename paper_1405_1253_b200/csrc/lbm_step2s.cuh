@@ -367,9 +367,9 @@ __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_cons
     __shared__ unsigned long long bars[2 * S::NRB + 2 * S::NST];
     const int tid = threadIdx.x;
     const int w = a.w;                                   // strips of w <= TX columns (w even: TMA boxes start on 16 bytes)
-    const int x0 = blockIdx.x * w, z0 = blockIdx.y * ZC;
+    const int x0 = blockIdx.x * w, z0 = a.zbase + blockIdx.y * ZC;   // a z-slab updates its own rows; its ghost rows are sources only
     const int ncols = min(w, a.Lx - x0);                // output columns of this strip
-    const int zend = min(a.Lz, z0 + ZC);                // output rows [z0, zend)
+    const int zend = min(a.zend, z0 + ZC);              // output rows [z0, zend)
     const int rlast = min(a.Lz, zend + 3);              // intermediate rows [max(0, z0-3), rlast)
     const int NP = (zend - z0 + S::R - 1) / S::R;       // consumer passes
     const unsigned bar_full = (unsigned)__cvta_generic_to_shared(&bars[0]);     // [NRB] ring rows written (producers -> consumers)

@@ -38,8 +38,10 @@ def exchange_messages(send_up, send_dn, recv_below, recv_above, rank: int, world
 
 
 class SlabRing:
-    """The slab of this rank plus its message buffers.  `step(n)`: per step, pack on the exchange stream, interior rows
-    on the main stream while the messages travel, unpack, edge rows (interior first)."""
+    """The slab of this rank plus its message buffers.  `step(n)`: pairs of steps with the two-step kernel (6 whole
+    ghost rows per open side and pair, exchanged before the launch: a few microseconds beside milliseconds), an odd
+    last step -- or every step with `fused=False` -- with the one-step kernel: pack on the exchange stream, interior
+    rows on the main stream while the messages travel, unpack, edge rows (interior first)."""
 
     def __init__(self, Lx: int, Lz: int, tau: float, g: float, rank: int, world: int, wall_kind: int = 0,
                  T_wall=(1.0, 1.0), device="cuda", group=None):
@@ -50,13 +52,28 @@ class SlabRing:
         self.z0, self.nz = partition(Lz, world)[rank]
         self.slab = Slab(Lx, Lz, self.z0, self.nz, tau, g, wall_kind=wall_kind, T_wall=T_wall, device=device)
         self.send_up, self.send_dn, self.recv_below, self.recv_above = (self.slab.new_message() for _ in range(4))
+        self.send2_up, self.send2_dn, self.recv2_below, self.recv2_above = (self.slab.new_message(True) for _ in range(4))
         self.xs = torch.cuda.Stream(device=self.slab.device)
 
-    def step(self, n: int = 1):
+    def step(self, n: int = 1, fused: bool = True):
         import torch
         s = self.slab
         main = torch.cuda.current_stream(s.device)
-        for _ in range(n):
+        pairs = n // 2 if fused else 0
+        for _ in range(pairs):
+            if s.open_above:
+                s.pack2(1, self.send2_up, stream=main)
+            if s.open_below:
+                s.pack2(0, self.send2_dn, stream=main)
+            for r in exchange_messages(self.send2_up, self.send2_dn, self.recv2_below, self.recv2_above, self.rank,
+                                       self.world, self.group):
+                r.wait()
+            if s.open_below:
+                s.unpack2(0, self.recv2_below, stream=main)
+            if s.open_above:
+                s.unpack2(1, self.recv2_above, stream=main)
+            s.step2(stream=main)
+        for _ in range(n - 2 * pairs):
             self.xs.wait_stream(main)
             with torch.cuda.stream(self.xs):
                 if s.open_above:

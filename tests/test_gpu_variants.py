@@ -179,6 +179,50 @@ def test_slabs_with_exchanged_ghost_rows_equal_the_whole_lattice(pkg, orc, Lx, L
     whole.close()
 
 
+def _run_slabs_fused(pkg, slabs, npairs):
+    """Pairs of steps with the two-step kernel: whole 6-row messages, device-to-device copies, one stream."""
+    import torch
+    up, dn, below, above = ([s.new_message(True) for s in slabs] for _ in range(4))
+    for _ in range(npairs):
+        for i, s in enumerate(slabs):
+            if s.open_above: s.pack2(1, up[i])
+            if s.open_below: s.pack2(0, dn[i])
+        for i, s in enumerate(slabs):
+            if s.open_below: below[i].copy_(up[i - 1], non_blocking=True); s.unpack2(0, below[i])
+            if s.open_above: above[i].copy_(dn[i + 1], non_blocking=True); s.unpack2(1, above[i])
+        for s in slabs:
+            s.step2()
+    torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("wall_kind", [0, 1])
+@pytest.mark.parametrize("Lx,Lz,cuts,n", [(64, 128, (0, 50, 128), 21), (130, 70, (0, 6, 30, 64, 70), 11), (33, 40, (0, 17, 40), 9),
+                                          (600, 300, (0, 100, 207, 300), 14)])
+def test_slabs_with_the_two_step_kernel_equal_the_whole_lattice(pkg, orc, Lx, Lz, cuts, n, wall_kind):
+    """z-slabs stepped two steps at a time (lbm_slab_pack2 / unpack2 / step2: 6 whole ghost rows with wrap columns), an
+    odd last step with the one-step slab path: bit-identical to the whole lattice, within the oracle tolerance; slabs
+    down to 6 rows, several strips, both wall kinds."""
+    import torch
+    f0 = _random_state(orc, Lx, Lz, 3 * Lx + 7 * Lz)
+    kw = dict(wall_kind=wall_kind, T_wall=(1.02, 0.97))
+    whole = pkg.Lattice(Lx, Lz, 0.75, 2e-4, **kw)
+    whole.set_variant(1)
+    whole.set_populations(torch.from_numpy(f0).cuda())
+    whole.step(n)
+    slabs = [pkg.Slab(Lx, Lz, z0, z1 - z0, 0.75, 2e-4, **kw) for z0, z1 in zip(cuts[:-1], cuts[1:])]
+    for s in slabs:
+        s.set_populations(torch.from_numpy(np.ascontiguousarray(f0[:, s.z0:s.z0 + s.nz])).cuda())
+    _run_slabs_fused(pkg, slabs, n // 2)
+    _run_slabs(pkg, slabs, n % 2)
+    got = torch.cat([s.get_populations() for s in slabs], dim=1)
+    assert torch.equal(got, whole.get_populations())
+    ref = orc.step(f0, 0.75, 2e-4, nsteps=n, wall_kind=wall_kind, T_bot=1.02, T_top=0.97)
+    assert _rel(got.cpu().numpy(), ref) < POP_RTOL
+    for s in slabs:
+        s.close()
+    whole.close()
+
+
 def test_slabs_rt_config_init_and_widths(pkg, orc):
     """lbm_init_rt on slabs uses global heights and fills the ghost rows; the mixing widths are partial sums."""
     cfg = si.scaled(si.rt_config(2), 128, 256)
