@@ -416,8 +416,10 @@ def run_slabs(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "Lx": cfg.Lx, "Lz": cfg.Lz, "tau": cfg.tau, "g": cfg.g,
-                       "parallelism": f"{world} z-slabs, 3 ghost rows per open side, 26 population-rows per message",
-                       "message_bytes": 26 * cfg.Lx * 8, "L_u": float(w[0]), "L_d": float(w[1])},
+                       "parallelism": f"{world} z-slabs; pairs of steps with the two-step kernel (6 whole ghost rows per open "
+                                      "side and pair), an odd step with the one-step kernel (26 population-rows, interior first)",
+                       "message2_bytes": 6 * 37 * (cfg.Lx + 16) * 8, "message_bytes": 26 * cfg.Lx * 8,
+                       "L_u": float(w[0]), "L_d": float(w[1])},
             "gpu_launches": launches, "clocks": clocks}))
     ring.close()
     dist.destroy_process_group()
