@@ -369,9 +369,10 @@ def run_ours(args):
 
 
 def run_slabs(args):
-    """--slabs under torchrun (N > 1): ONE lattice (the N = 1 workload) cut into z-slabs, one per rank, 26
-    population-rows exchanged per open side and step over NCCL, hidden behind the interior rows (SURVEY 8(f)4;
-    PAPER.md:110, 116-118).  Strong scaling: value = sites x steps / max-over-ranks time.  Not the default N > 1 mode
+    """--slabs under torchrun (N > 1): ONE lattice (the N = 1 workload) cut into z-slabs, one per rank, ghost rows
+    exchanged over NCCL point-to-point calls (SlabRing: 6 whole rows per pair of steps for the two-step kernel; 26
+    population-rows per step, hidden behind the interior rows, for an odd step -- SURVEY 8(f)4; PAPER.md:110,
+    116-118).  Strong scaling: value = sites x steps / max-over-ranks time.  Not the default N > 1 mode
     (north_star fixes one GPU: the default is independent replicas); unmeasured on hardware in this run (one GPU per
     call), verified on one GPU by tests/test_gpu_variants.py (slabs on one device, bit-identical to the whole lattice)."""
     import torch
