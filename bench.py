@@ -34,7 +34,7 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # (workload, steps per launch, strip width, rows per chunk) is the one that was captured; null otherwise.
 NCU_TRAFFIC = {
     ("rt_single_4096x8192", 1, None, None): (19.839e9, "profiles/r2_step_kernels_full.md"),
-    ("rt_single_4096x8192", 2, 56, 410): (20.181e9, "profiles/r2_step2s_kernel_full.md"),
+    ("rt_single_4096x8192", 2, 56, 410): (20.203e9, "profiles/r2_step2s_kernel_full.md"),
 }
 
 
