@@ -2,10 +2,11 @@
 // the intermediate lattice f1 = step(f0) kept in shared memory, so that HBM sees ~296 B read + 296 B written per
 // site per TWO steps instead of per step.  Warp-specialised: loader / producer / consumer warps.
 //
-// A block owns a strip of TX output columns and marches up a chunk of ZC rows, R rows per pass.
+// A block owns a strip of w <= TX output columns (w a launch argument) and marches up a chunk of ZC rows of the row
+// range [zbase, zend) (the whole lattice, or the own rows of a z-slab whose ghost rows are sources only), R rows per pass.
 //   loader (1 warp)   the gather part of the first step: seven TMA tensor box loads per pass (one per e_z) bring the
 //                     source rows of the pass into a shared-memory STAGE, NST passes ahead;
-//   producers         one thread per site of the R x (TX+6) intermediate slab (three halo columns per side are
+//   producers         one thread per site of the R x (w+6) intermediate slab (three halo columns per side are
 //                     recomputed, not exchanged): read the 37 populations from the stage with the e_x shift, collide
 //                     in registers, store f1 into the RING;
 //   consumers         one thread per output site: gather the 37 populations from ring rows k-3..k+3, collide, write
@@ -16,7 +17,7 @@
 // row picture of DESIGN.md reading 9), written by the producers of those rows, so the consumers' gather is uniform
 // there; at the top wall the mirror rows are still resident and the consumers remap indices.  Periodic x (a1): every
 // row is stored with XH spare columns on either side, of which the nearest XW hold the periodic images (written by
-// the consumers of the seam strips, or refreshed by wrap_columns_kernel after any other writer), so the boxes of the
+// spare consumer lanes of the seam strips, or refreshed by wrap_columns_kernel after any other writer), so the boxes of the
 // seam strips need no special case -- a per-thread global gather for the seam sites cost a factor of two on
 // single-wave launches (profiles/r2_two_step.md).  Sites whose first-step sources reflect (wall rows) are gathered
 // from global memory by their producer thread; the TMA unit zero-fills those parts of the boxes (rows outside the
@@ -127,8 +128,8 @@ struct Step2sShape {
 //   <60,2,3,0> 15.7         (5 producer warps again)
 //   <64,2,1,1> 14.2, <64,3,1,0> 14.7   one stage buffer: the producers wait for the TMA round trip
 //   <112,1,2,0> 16.8, <120,1,1,0> 14.8  one row per pass, wide strips (5 % halo work instead of 11 %), fewer buffers
-//   <58,2,3,0> with the strip width a launch argument (round 2): 64 producer lanes per intermediate row, so no warp
-//                           straddles two rows; the host picks an even width <= 58 that divides Lx without a sliver
+// Round 2: the strip width is a launch argument w <= TX (a multiple of 4, chosen by the host so that the strips divide
+// Lx without a sliver); 64 producer lanes per intermediate row whatever w, so no warp straddles two rows.
 #ifndef S2S_TX   // shape experiments: -DS2S_TX=.. -DS2S_R=.. -DS2S_NST=.. -DS2S_SL=..
 #define S2S_TX 56
 #define S2S_R 2
@@ -137,7 +138,7 @@ struct Step2sShape {
 #endif
 using Step2sWide = Step2sShape<S2S_TX, S2S_R, S2S_NST, S2S_SL>;
 
-// Tensor maps of the source lattice (host-encoded, lbm_api.cu): rank 3 (x: Lx, z: Lz, l: 37), strides
+// Tensor maps of the source lattice (host-encoded, lbm_api.cu): rank 3 (x: XH + Lx + XH stored columns, z: stored rows, l: 37), strides
 // (pitch, plane) doubles, box (SP, R, n) for n = 3, 5, 7 -- the populations with the same e_z are consecutive in l.
 struct Step2sMaps {
     alignas(64) unsigned char m[3][128];                // CUtensorMap x 3 (box depth 3, 5, 7 populations)
