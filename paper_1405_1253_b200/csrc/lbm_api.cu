@@ -191,11 +191,12 @@ lbm::StepArgs step_args(const lbm_t *h)
 
 // Launch plan of lbm_step for this lattice.  The two-step kernel runs strips of w <= TX columns in chunks of ZC rows,
 // one block per SM at a time, every block (ZC + 6)/R passes of about the same duration: the plan minimises
-//   (waves + 0.3) x (ZC + 6 + fill),  waves = ceil(strips x chunks / SMs)
+//   (waves + 0.15) x (ZC + 6 + fill) x (1 + ZC/16000),  waves = ceil(strips x chunks / SMs),  fill = 10 rows' worth
 // over the strip count and ZC (whole waves: no tail; few chunks: little warm-up -- a chunk recomputes the 6
-// intermediate rows below it; + 0.3: the blocks of a wave do not finish together -- wall chunks gather three rows
-// from global memory -- so a launch of few long waves waits for its slowest block), and takes the one-step kernel
-// where that is predicted to be faster (small lattices).  Measurements: profiles/r2_two_step.md.
+// intermediate rows below it and waits for its first boxes; + 0.15: the blocks of a wave do not finish together --
+// wall chunks gather three rows from global memory -- so a launch waits for its slowest block), and takes the
+// one-step kernel where that is predicted to be faster (small lattices).  Constants fitted to the chunk-size runs of
+// profiles/r2_two_step.md section 3.
 const lbm_plan &make_plan(lbm_t *h)
 {
     using S2 = lbm::Step2sWide;
@@ -217,20 +218,22 @@ const lbm_plan &make_plan(lbm_t *h)
             if (ZC < 6) ZC = 6;
             const int nch = (Lz + ZC - 1) / ZC;
             const long long waves = ((long long)strips * nch + sms - 1) / sms;
-            const double cost = ((double)waves + 0.3) * (ZC + 6 + 4);   // + 4: pipeline fill of a block (first TMA round trip)
+            // x (1 + ZC / 16000): blocks that march for thousands of rows drift apart, and the columns two neighbouring
+            // strips both load stop meeting in L2 (4096x8192 in one wave of 4096-row chunks: -6 %)
+            const double cost = ((double)waves + 0.15) * (ZC + 6 + 10) * (1.0 + ZC / 16000.0);
             if (cost < best - 1e-9) { best = cost; p.w = w; p.strips = strips; p.ZC = ZC; p.chunks = nch; }
         }
     }
     if (h->zchunk > 0) {                                      // rows per block forced (tests, experiments)
         p.ZC = h->zchunk;
         p.chunks = (Lz + p.ZC - 1) / p.ZC;
-        best = ((double)(((long long)p.strips * p.chunks + sms - 1) / sms) + 0.3) * (p.ZC + 10);
+        best = ((double)(((long long)p.strips * p.chunks + sms - 1) / sms) + 0.15) * (p.ZC + 16) * (1.0 + p.ZC / 16000.0);
     }
     // predicted time of two steps, microseconds: the two-step kernel spends ~0.65-0.7 us per unit of the cost above
     // on lattices of up to a few million sites (1.3-1.4 us per pass of two rows; the largest lattices, DRAM- and
     // power-bound, need 0.9) plus ~4 us per launch; the one-step kernel ~92 ps per site and step plus ~3 us per launch
     // (profiles/r2_sweep.md)
-    const double t_fused = 0.70 * best + 4.0;
+    const double t_fused = 0.66 * best + 4.0;
     const double t_single = 2.0 * (92e-6 * (double)Lx * Lz + 3.0);
     const bool can_fuse = h->tma_ok && !h->inplace;
     p.fused = can_fuse && (h->variant == 3 || (h->variant == 0 && t_fused < t_single));
