@@ -649,12 +649,18 @@ int lbm_step(lbm_t *h, int n, void *stream)
         const void *fn = h->persist_tb == 64
                              ? (h->wall_kind == 1 ? (const void *)lbm::step_persistent_kernel<64, true> : (const void *)lbm::step_persistent_kernel<64, false>)
                              : (h->wall_kind == 1 ? (const void *)lbm::step_persistent_kernel<128, true> : (const void *)lbm::step_persistent_kernel<128, false>);
-        CUDA_TRY(cudaLaunchCooperativeKernel(fn, dim3(h->persist_blocks), dim3(h->persist_tb), args, 0, st));
-        h->launches++;
-        h->wrap_ok[0] = h->wrap_ok[1] = false;
-        if (n % 2) h->cur ^= 1;
-        h->steps += n;
-        return LBM_OK;
+        if (cudaLaunchCooperativeKernel(fn, dim3(h->persist_blocks), dim3(h->persist_tb), args, 0, st) == cudaSuccess) {
+            h->launches++;
+            h->wrap_ok[0] = h->wrap_ok[1] = false;
+            if (n % 2) h->cur ^= 1;
+            h->steps += n;
+            return LBM_OK;
+        }
+        // the grid is not co-resident after all (a shared or partitioned GPU): launched steps from now on, outside capture
+        cudaGetLastError();
+        h->persist_blocks = 0;
+        if (cap != cudaStreamCaptureStatusNone && n % 2)
+            return fail(LBM_ERR_INVALID, "lbm_step: %d launched steps cannot be captured (odd number of swaps)", n);
     }
     int s = 0;
     if (plan.fused && n >= 2) {
