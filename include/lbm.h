@@ -194,6 +194,34 @@ int lbm_totals(lbm_t *h, double *out4, void *stream);
 int lbm_diagnostics(lbm_t *h, double T_d, double T_m, double T_u, double *widths2, double *totals4, double *Tbar,
                     double *Trms, double *Ekbar, double *Ekrms, void *stream);
 
+/* The widths, totals and Tbar of lbm_diagnostics for callers that are not allowed to allocate device memory.
+ * Who that is: a program whose GPU memory is handed out once by a pool it does not control (a framework's caching
+ * allocator, a job that was given a fixed carve-out), where a cudaMalloc behind the pool's back can make the pool run
+ * out later; and a probe that is called from inside another code's time loop, where cudaMalloc would stall every
+ * stream of the device.  lbm_create allocates the handle's scratch, so such a caller has no handle: this call takes
+ * the population buffer itself and keeps its scratch (the per-row partial results, eq. 12 / PAPER.md:128, 183-186) in
+ * a static device array inside the library, 8 x LBM_NOALLOC_MAX_ROWS doubles = 1 MiB, which every GPU that loads the
+ * library holds until the process exits.  It calls no cudaMalloc / cudaFree and no allocating library routine.
+ *   pop_buf     DEVICE: a lattice copy exactly as handed to lbm_create (pop_buf0 / pop_buf1), buf_bytes long, 256-byte
+ *               aligned, holding the current state of an Lx x Lz lattice in the ordinary layout (a two-copy handle's
+ *               current copy, or an in-place handle after an even number of steps).  Read only.
+ *   g           gravity of eq. 3 (the hydrodynamic T^(H), u^(H) of PAPER.md:94 need it).
+ *   result6_dev DEVICE out[6]: L_u, L_d (eq. 12; both 0 if T_d == T_m or T_m == T_u), sum f, sum c_x f, sum c_z f,
+ *               sum |c|^2 f.  Tbar_dev: DEVICE out[Lz] or NULL, Tbar(k) of PAPER.md:128.
+ * Asynchronous on `stream`; nothing is synchronised, the outputs are valid once the stream reaches that point.
+ * Limit: Lz <= LBM_NOALLOC_MAX_ROWS, else LBM_ERR_INVALID with a message naming the limit (Lx is not limited).
+ * Other errors: null / misaligned / undersized buffer, Lx < 7, Lz < 6 (LBM_ERR_INVALID, checked before any device
+ * work); no sm_100 device current (LBM_ERR_NODEVICE); a failed launch or cudaGetSymbolAddress (LBM_ERR_CUDA).
+ * First call on a device: looks up the device address of the static array (cudaGetSymbolAddress, with that device
+ * current) and remembers it per device; make that first call before any stream capture begins.
+ * Sharing: all calls on one GPU use the same array, and it keeps the previous call's contents.  The part a call uses
+ * is cleared and rewritten by that call on its stream, so calls that follow each other on one stream are independent
+ * of each other; two calls whose work may overlap on the GPU (different streams, different host threads) race on the
+ * array and give undefined results -- order them with an event or use one stream. */
+#define LBM_NOALLOC_MAX_ROWS 16384
+int lbm_diagnostics_noalloc(const void *pop_buf, size_t buf_bytes, int Lx, int Lz, double g, double T_d, double T_m,
+                            double T_u, double *result6_dev, double *Tbar_dev, void *stream);
+
 /* Scales of a Rayleigh-Taylor run (host arithmetic): Atwood number At = (T_d - T_u)/(T_d + T_u) (Table II,
  * PAPER.md:144) and tau_RT = sqrt(Lx / (g At)), Lx in sites.  HOST outputs, any may be NULL. */
 int lbm_rt_scales(double Lx, double g, double T_d, double T_u, double *At, double *tau_rt);

@@ -12,7 +12,7 @@ from . import binding
 from .binding import LbmError, NPOP, lbm_params, lbm_rt_init
 
 __all__ = ["Lattice", "Slab", "LbmError", "NPOP", "buffer_bytes", "slab_buffer_bytes", "tables", "growth_rate",
-           "rt_scales", "fp64_peak"]
+           "rt_scales", "fp64_peak", "diagnostics_noalloc"]
 
 
 def buffer_bytes(Lx: int, Lz: int) -> int:
@@ -58,6 +58,26 @@ def _stream_ptr(stream, device=None):
     import torch
     s = stream if stream is not None else torch.cuda.current_stream(device)
     return C.c_void_p(s.cuda_stream)
+
+
+def diagnostics_noalloc(pop_buf, Lx: int, Lz: int, g: float, T_d: float, T_m: float, T_u: float, result6, Tbar=None,
+                        stream=None):
+    """lbm_diagnostics_noalloc: mixing widths, lattice totals and Tbar of a lattice copy, for callers that must not
+    allocate device memory (their memory comes from a pool that cudaMalloc would bypass, or they run inside another
+    code's time loop, which a cudaMalloc would stall).  Nothing is allocated here either: `pop_buf` is the float64 CUDA
+    tensor that holds the lattice copy (what lbm_create was given), `result6` a float64 CUDA tensor of 6 entries
+    (L_u, L_d, sum f, sum c_x f, sum c_z f, sum |c|^2 f) and `Tbar` an optional one of Lz entries, all owned by the
+    caller.  The scratch is a 1 MiB static array inside the library, shared by every call on that GPU: Lz may be at
+    most binding.NOALLOC_MAX_ROWS, and calls that can overlap on the GPU (different streams) race.  Asynchronous."""
+    import torch
+    for t, n, name in ((result6, 6, "result6"), (Tbar, Lz, "Tbar")):
+        if t is not None and (not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or t.numel() < n
+                              or t.device != pop_buf.device):
+            raise LbmError(f"{name} must be a contiguous float64 CUDA tensor of at least {n} entries on the lattice's device")
+    with torch.cuda.device(pop_buf.device):
+        binding.check(binding.load().lbm_diagnostics_noalloc(
+            _dptr(pop_buf), pop_buf.numel() * pop_buf.element_size(), int(Lx), int(Lz), float(g), float(T_d), float(T_m),
+            float(T_u), _dptr(result6), _dptr(Tbar), _stream_ptr(stream, pop_buf.device)))
 
 
 def _on_device(method):

@@ -12,6 +12,7 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblbm_b200.so")
 NPOP = 37
+NOALLOC_MAX_ROWS = 16384   # LBM_NOALLOC_MAX_ROWS of include/lbm.h
 
 # every symbol include/lbm.h declares
 SYMBOLS = [
@@ -21,6 +22,7 @@ SYMBOLS = [
     "lbm_layout", "lbm_kernel_launches", "lbm_fp64_peak", "lbm_set_variant", "lbm_set_zchunk", "lbm_get_plan", "lbm_tables", "lbm_last_error",
     "lbm_diagnostics", "lbm_rt_scales", "lbm_slab_buffer_bytes", "lbm_create_slab", "lbm_slab_info", "lbm_slab_pack",
     "lbm_slab_unpack", "lbm_slab_step", "lbm_get_window", "lbm_slab_pack2", "lbm_slab_unpack2", "lbm_slab_step2",
+    "lbm_diagnostics_noalloc",
 ]
 
 
@@ -91,6 +93,8 @@ def load():
     L.lbm_slab_unpack.argtypes = [vp, C.c_int, vp, vp]
     L.lbm_slab_step.argtypes = [vp, C.c_int, vp]
     L.lbm_get_window.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
+    L.lbm_diagnostics_noalloc.argtypes = [vp, C.c_size_t, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double,
+                                          vp, vp, vp]
     for name in SYMBOLS:
         if name not in ("lbm_buffer_bytes", "lbm_slab_buffer_bytes", "lbm_last_error"):
             getattr(L, name).restype = C.c_int

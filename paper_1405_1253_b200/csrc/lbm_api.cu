@@ -8,6 +8,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -989,3 +990,83 @@ int lbm_set_variant(lbm_t *h, int variant)
 }
 
 }  // extern "C"
+
+// ---- lbm_diagnostics_noalloc: the diagnostics pass for callers that may not allocate -------------------------------
+// Who needs this: code that runs where cudaMalloc is off limits.  Typical cases are a host program whose device memory
+// is handed out once by a framework's pool (anything cudaMalloc takes behind the pool's back can push the pool over the
+// edge later, and cudaMalloc also synchronises the whole device, which stalls every other stream of a running job), and
+// a monitoring hook that is called in the middle of somebody else's time loop and must not disturb its memory or its
+// timing.  Such a caller cannot use lbm_create at all (it allocates the handle's scratch), so this entry point takes the
+// raw population buffer instead of a handle.
+//
+// The per-row array that row_diagnostics_kernel writes and final_diagnostics_kernel reads lives in the library image:
+// 8 x LBM_NOALLOC_MAX_ROWS doubles = 1 MiB, resident on every GPU that loads liblbm_b200.so until the process exits.
+// `g_noalloc_rows` is a device symbol.  On the host its name is only a stand-in (taking its address in host code gives a
+// host address a kernel must never see), so the device address is asked for once per device with cudaGetSymbolAddress
+// (noalloc_rows_of_current_device) and that pointer is what the kernels get.
+static __device__ __align__(256) double g_noalloc_rows[8 * LBM_NOALLOC_MAX_ROWS];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mu;
+double *g_noalloc_ptr[NOALLOC_MAX_DEVICES];    // device address of g_noalloc_rows on device d; null = not set up yet
+
+// Set-up, once per device, with that device current: architecture check and the device address of the static array.
+int noalloc_rows_of_current_device(double **rows)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return fail(LBM_ERR_NODEVICE, "lbm_diagnostics_noalloc: no CUDA device"); }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES)
+        return fail(LBM_ERR_INVALID, "lbm_diagnostics_noalloc: device ordinal %d is beyond the %d this entry point keeps track of", dev, NOALLOC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        int major = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(LBM_ERR_NODEVICE, "lbm_diagnostics_noalloc: cannot query device %d", dev);
+        }
+        if (major != 10) return fail(LBM_ERR_NODEVICE, "lbm_diagnostics_noalloc: built for sm_100a, device %d is sm_%dx", dev, major);
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_rows);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(LBM_ERR_CUDA, "lbm_diagnostics_noalloc: cudaGetSymbolAddress(g_noalloc_rows) on device %d: %s", dev,
+                        e != cudaSuccess ? cudaGetErrorString(e) : "null address");
+        }
+        g_noalloc_ptr[dev] = (double *)p;
+    }
+    *rows = g_noalloc_ptr[dev];
+    return LBM_OK;
+}
+
+}  // namespace
+
+extern "C" int lbm_diagnostics_noalloc(const void *pop_buf, size_t buf_bytes, int Lx, int Lz, double g, double T_d, double T_m,
+                                       double T_u, double *result6_dev, double *Tbar_dev, void *stream)
+{
+    // argument checks first: they need no device, and an oversized lattice must never reach the fixed-size array
+    if (!pop_buf || !result6_dev) return fail(LBM_ERR_INVALID, "lbm_diagnostics_noalloc: pop_buf and result6_dev are required");
+    if (Lx < 7 || Lz < 6) return fail(LBM_ERR_INVALID, "lbm_diagnostics_noalloc: need Lx >= 7 and Lz >= 6 (got %d x %d)", Lx, Lz);
+    if (Lz > LBM_NOALLOC_MAX_ROWS)
+        return fail(LBM_ERR_INVALID, "lbm_diagnostics_noalloc: Lz = %d rows exceed LBM_NOALLOC_MAX_ROWS = %d, the size of the "
+                    "static scratch array; use lbm_create + lbm_diagnostics for taller lattices", Lz, LBM_NOALLOC_MAX_ROWS);
+    if ((uintptr_t)pop_buf & 255) return fail(LBM_ERR_INVALID, "lbm_diagnostics_noalloc: pop_buf must be 256-byte aligned");
+    const size_t need = (size_t)plane_of(Lx, Lz) * LBM_NPOP * sizeof(double);
+    if (buf_bytes < need) return fail(LBM_ERR_INVALID, "lbm_diagnostics_noalloc: the buffer has %zu bytes, a %d x %d lattice needs %zu", buf_bytes, Lx, Lz, need);
+    double *rows = nullptr;
+    int rc = noalloc_rows_of_current_device(&rows);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const lbm::Layout lay{Lx, Lz, pitch_of(Lx), plane_of(Lx, Lz), 0, Lz, false};
+    // The array still holds what the previous call left there.  Every entry the second kernel reads is rewritten by the
+    // first one, so a correct run never depends on old contents; the part this call uses is zeroed all the same, so that
+    // a row kernel that did not run cannot pass the last lattice's numbers off as this one's.
+    CUDA_TRY(cudaMemsetAsync(rows, 0, sizeof(double) * 8 * (size_t)Lz, st));
+    lbm::row_diagnostics_kernel<false><<<Lz, lbm::RED_T, 0, st>>>((const double *)pop_buf + lbm::XH, lay, g, rows);
+    CUDA_TRY(cudaGetLastError());
+    lbm::final_diagnostics_kernel<<<1, lbm::RED_T, 0, st>>>(rows, Lz, T_d, T_m, T_u, result6_dev);
+    CUDA_TRY(cudaGetLastError());
+    if (Tbar_dev) CUDA_TRY(cudaMemcpyAsync(Tbar_dev, rows, sizeof(double) * (size_t)Lz, cudaMemcpyDeviceToDevice, st));
+    return LBM_OK;
+}
