@@ -164,6 +164,12 @@ __global__ void __launch_bounds__(TX *TZ, 512 / (TX * TZ)) step_kernel_site(cons
 // global memory, polled with acquire loads; the block barrier before it and the fence make the block's stores
 // visible).  Loads bypass L1 (the other copy was rewritten by other SMs a moment ago).  Same gather, same collision:
 // bit-identical to n launches of the one-step kernel.
+// The counter only grows.  The host sets it to BARRIER_START = 0xFFFFFFFF before every launch (a byte memset of 0xFF),
+// so EVERY launch takes the counter through the 32-bit wrap at its first barrier, and the wait compares the signed
+// distance to the target, which is right across the wrap as long as a launch adds fewer than 2^31 arrivals:
+// lbm_step issues at most PERSIST_MAX_STEPS steps per launch (2^20 steps x at most a few hundred blocks < 2^29).
+constexpr unsigned BARRIER_START = 0xFFFFFFFFu;
+constexpr int PERSIST_MAX_STEPS = 1 << 20;
 template <int TB, bool ISO>
 __global__ void __launch_bounds__(TB) step_persistent_kernel(StepArgs a, double *buf0, double *buf1, int cur, const int nsteps,
                                                              unsigned *counter)
@@ -186,11 +192,11 @@ __global__ void __launch_bounds__(TB) step_persistent_kernel(StepArgs a, double 
             if (threadIdx.x == 0) {
                 __threadfence();
                 atomicAdd(counter, 1u);
-                const unsigned target = (unsigned)(s + 1) * gridDim.x;
+                const unsigned target = BARRIER_START + (unsigned)(s + 1) * gridDim.x;     // modulo 2^32
                 unsigned seen;
                 do {
                     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
-                } while (seen < target);
+                } while ((int)(seen - target) < 0);
             }
             __syncthreads();
         }
