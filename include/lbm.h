@@ -84,8 +84,9 @@ typedef struct {
 /* Bytes each population buffer must have for an Lx x Lz lattice (padded rows, 37 planes); 0 if invalid. */
 size_t lbm_buffer_bytes(int Lx, int Lz);
 
-/* Creates a handle. Errors: Lx < 7, Lz < 6, tau <= 0.5, g < 0, wall_kind not 0/1, wall temperatures <= 0 with
- * wall_kind 1, null pop_buf0 / misaligned / undersized buffers, no sm_100 device.  *out is set to NULL on failure. */
+/* Creates a handle. Errors: Lx < 7, Lz < 6, Lz > 65535 (stored rows, a slab's ghost rows included: the kernels put
+ * rows on grid.y), tau <= 0.5, g < 0, wall_kind not 0/1, wall temperatures <= 0 with wall_kind 1, null pop_buf0 /
+ * misaligned / undersized buffers, no sm_100 device.  *out is set to NULL on failure. */
 int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p);
 
 /* ---- z-slabs: the lattice split along z over several handles (one per GPU), SURVEY 8(f)4.  The paper splits
@@ -140,7 +141,8 @@ int lbm_init_equilibrium(lbm_t *h, const double *rho, const double *ux, const do
                          void *stream);
 
 /* Canonical dense [37][Lz][Lx] populations <-> the library's layout. `f` is a DEVICE pointer
- * (lbm_*_populations) or a HOST pointer (lbm_*_populations_host; these synchronise the stream). */
+ * (lbm_*_populations) or a HOST pointer (lbm_*_populations_host; these synchronise the stream, stage through the
+ * other lattice copy and are refused, LBM_ERR_INVALID, on a slab between lbm_slab_step(INTERIOR) and (EDGES)). */
 int lbm_set_populations(lbm_t *h, const double *f_dev, void *stream);
 int lbm_get_populations(lbm_t *h, double *f_dev, void *stream);
 int lbm_set_populations_host(lbm_t *h, const double *f_host, void *stream);
@@ -245,7 +247,7 @@ int lbm_fp64_peak(double *tflops, int iters, void *stream);
  * predicted faster than two single steps (from about 512x512 up), one cooperative launch for all n steps on
  * lattices of at most ~37 000 sites (persistent kernel with a grid barrier between steps), else one step per
  * launch; 1 one step per launch (256-thread blocks), 2 one step (128), 3 two steps per launch forced
- * (LBM_ERR_CUDA from lbm_step for in-place handles: it needs two copies).  All give bit-identical results. */
+ * (LBM_ERR_INVALID from lbm_step for in-place handles: it needs two copies).  All give bit-identical results. */
 int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kernel (>= 3), or 0 = automatic */
 /* The launch plan lbm_step uses for this lattice with the current variant / zchunk settings (HOST outputs, any may

@@ -127,6 +127,8 @@ struct lbm_handle {
     double *buf[2];        // site (0,0) of population 0 in each copy (ubuf + XH); buf[1] = null: in-place, one copy
     bool inplace, layout_m;   // in-place path: layout_m after an odd number of steps (lbm_step.cuh)
     bool wrap_ok[2];       // the wrap columns of copy i hold the periodic images of its current contents
+    bool cap_seen;         // refresh_wrap_columns: the last stream capture that recorded a refresh
+    unsigned long long cap_id;
     // z-slab (lbm_create_slab): height of the whole lattice, first own global row, own rows, ghost rows below / above
     bool slab;
     int Lz_glob, z0, nz, glo, ghi;
@@ -245,7 +247,15 @@ const lbm_plan &make_plan(lbm_t *h)
 // periodic images for the two-step kernel's boxes (a1), if copy `i` was last written by anything but that kernel
 int refresh_wrap_columns(lbm_t *h, int i, cudaStream_t st)
 {
-    if (h->wrap_ok[i]) return LBM_OK;
+    // Under stream capture the refresh is always recorded: a replay may follow lbm_set_populations / lbm_init_*, whose
+    // writes leave the wrap columns stale, and the graph must not depend on what wrap_ok said at capture time.
+    // Once per capture is enough: later launches of the same capture read rows the two-step kernel itself wrote.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    unsigned long long cap_id = 0;
+    if (cudaStreamGetCaptureInfo(st, &cap, &cap_id) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+    const bool first_of_capture = cap != cudaStreamCaptureStatusNone && (!h->cap_seen || h->cap_id != cap_id);
+    if (first_of_capture) { h->cap_seen = true; h->cap_id = cap_id; }
+    if (h->wrap_ok[i] && !first_of_capture) return LBM_OK;
     lbm::wrap_columns_kernel<lbm::XW><<<h->Lz, 2 * lbm::XW * LBM_NPOP, 0, st>>>(h->buf[i], h->layout());
     LAUNCHED(h);
     h->wrap_ok[i] = true;
@@ -359,7 +369,7 @@ int create_common(lbm_t **out, int Lx, int rows_stored, const lbm_params *p, con
     h->buf[0] = h->ubuf[0] + lbm::XH;
     h->buf[1] = h->ubuf[1] ? h->ubuf[1] + lbm::XH : nullptr;
     h->inplace = h->ubuf[1] == nullptr; h->layout_m = false;
-    h->wrap_ok[0] = h->wrap_ok[1] = false;
+    h->wrap_ok[0] = h->wrap_ok[1] = false; h->cap_seen = false; h->cap_id = 0;
     h->slab = false; h->Lz_glob = rows_stored; h->z0 = 0; h->nz = rows_stored; h->glo = h->ghi = 0; h->slab_phase = 0;
     h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 0; h->scratch = nullptr; h->plane_stage = nullptr;
     h->plan = lbm_plan{};
@@ -370,7 +380,7 @@ int create_common(lbm_t **out, int Lx, int rows_stored, const lbm_params *p, con
     return LBM_OK;
 }
 
-int finish_create(lbm_t **out)
+int finish_create(lbm_t **out, const char *fn)
 {
     lbm_handle *h = *out;
     if (!h->inplace) {
@@ -403,9 +413,11 @@ int finish_create(lbm_t **out)
     }
     cudaError_t e = cudaMalloc(&h->scratch, sizeof(double) * (8LL * h->nz + 8 + 2LL * h->Lx));
     if (e != cudaSuccess) {
-        delete h;
+        cudaGetLastError();
+        h->scratch = nullptr;
+        lbm_destroy(h);                  // frees the barrier counter too
         *out = nullptr;
-        return fail(LBM_ERR_CUDA, "lbm_create: cudaMalloc scratch: %s", cudaGetErrorString(e));
+        return fail(LBM_ERR_CUDA, "%s: cudaMalloc scratch: %s", fn, cudaGetErrorString(e));
     }
     return LBM_OK;
 }
@@ -445,7 +457,7 @@ size_t lbm_buffer_bytes(int Lx, int Lz)
 
 size_t lbm_slab_buffer_bytes(int Lx, int Lz_global, int z0, int nz)
 {
-    if (Lx < 7 || Lz_global < 6 || z0 < 0 || nz < GHOST || z0 + nz > Lz_global) return 0;
+    if (Lx < 7 || Lz_global < 6 || z0 < 0 || nz < 2 * GHOST || z0 + nz > Lz_global) return 0;   // as lbm_create_slab
     const int rows = nz + (z0 > 0 ? GHOST_STORED : 0) + (z0 + nz < Lz_global ? GHOST_STORED : 0);
     return rows < 6 ? 0 : (size_t)plane_of(Lx, rows) * LBM_NPOP * sizeof(double);
 }
@@ -465,7 +477,7 @@ int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p)
 {
     int rc = create_common(out, Lx, Lz, p, "lbm_create");
     if (rc) return rc;
-    return finish_create(out);
+    return finish_create(out, "lbm_create");
 }
 
 int lbm_create_slab(lbm_t **out, int Lx, int Lz_global, int z0, int nz, const lbm_params *p)
@@ -480,7 +492,7 @@ int lbm_create_slab(lbm_t **out, int Lx, int Lz_global, int z0, int nz, const lb
     if (rc) return rc;
     lbm_handle *h = *out;
     h->slab = true; h->Lz_glob = Lz_global; h->z0 = z0; h->nz = nz; h->glo = glo; h->ghi = ghi;
-    return finish_create(out);
+    return finish_create(out, "lbm_create_slab");
 }
 
 int lbm_destroy(lbm_t *h)
@@ -571,6 +583,9 @@ int lbm_set_populations_host(lbm_t *h, const double *f_host, void *stream)
 {
     NEED(h);
     if (!f_host) return fail(LBM_ERR_INVALID, "lbm_set_populations_host: null pointer");
+    // two-copy handles stage through the OTHER lattice copy, which holds the interior rows of a half-done slab step
+    if (h->slab && h->slab_phase != 0)
+        return fail(LBM_ERR_INVALID, "lbm_set_populations_host: a slab step is half done (interior launched, edges pending); finish it first");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t plane_elems = (size_t)h->Lx * h->nz;
     if (!h->inplace) {
@@ -598,6 +613,9 @@ int lbm_get_populations_host(lbm_t *h, double *f_host, void *stream)
 {
     NEED(h);
     if (!f_host) return fail(LBM_ERR_INVALID, "lbm_get_populations_host: null pointer");
+    // two-copy handles stage through the OTHER lattice copy, which holds the interior rows of a half-done slab step
+    if (h->slab && h->slab_phase != 0)
+        return fail(LBM_ERR_INVALID, "lbm_get_populations_host: a slab step is half done (interior launched, edges pending); finish it first");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t plane_elems = (size_t)h->Lx * h->nz;
     if (!h->inplace) {
@@ -631,8 +649,8 @@ int lbm_step(lbm_t *h, int n, void *stream)
     using S2 = lbm::Step2sWide;
     const lbm_plan &plan = make_plan(h);
     if (h->variant == 3 && !plan.fused)
-        return fail(LBM_ERR_CUDA, "lbm_step: the two-step kernel needs two lattice copies and tensor maps%s",
-                    h->tma_ok ? "" : " (cuTensorMapEncodeTiled failed)");
+        return fail(h->inplace ? LBM_ERR_INVALID : LBM_ERR_CUDA, "lbm_step: the two-step kernel needs two lattice copies and tensor maps%s",
+                    h->inplace || h->tma_ok ? "" : " (cuTensorMapEncodeTiled failed)");
     const bool persistent = h->persist_blocks > 0 && h->variant == 0 && !plan.fused && n >= 2;
     // Under stream capture the handle's bookkeeping (which copy is current) advances at capture time, not at replay:
     // a captured sequence must leave the current copy / layout where it was, i.e. swap the copies an even number of times.
@@ -643,22 +661,34 @@ int lbm_step(lbm_t *h, int n, void *stream)
         return fail(LBM_ERR_INVALID, "lbm_step: %d steps swap the lattice copies %d times here; a captured sequence must "
                     "swap them an even number of times (the ping-pong must return to the same copy)", n, swaps);
     if (persistent) {       // small lattice: all n steps in one cooperative launch (lbm_step.cuh)
-        CUDA_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(unsigned), st));
-        double *b0 = h->buf[0], *b1 = h->buf[1];
-        int cur = h->cur, nn = n;
-        void *args[] = {&a, &b0, &b1, &cur, &nn, &h->d_counter};
         const void *fn = h->persist_tb == 64
                              ? (h->wall_kind == 1 ? (const void *)lbm::step_persistent_kernel<64, true> : (const void *)lbm::step_persistent_kernel<64, false>)
                              : (h->wall_kind == 1 ? (const void *)lbm::step_persistent_kernel<128, true> : (const void *)lbm::step_persistent_kernel<128, false>);
-        if (cudaLaunchCooperativeKernel(fn, dim3(h->persist_blocks), dim3(h->persist_tb), args, 0, st) == cudaSuccess) {
-            h->launches++;
-            h->wrap_ok[0] = h->wrap_ok[1] = false;
-            if (n % 2) h->cur ^= 1;
-            h->steps += n;
-            return LBM_OK;
+        // ... in launches of at most PERSIST_MAX_STEPS steps: the barrier counter must not run a whole 2^31 ahead
+        bool launched = true;
+        cudaError_t le = cudaSuccess;
+        while (n > 0 && launched) {
+            double *b0 = h->buf[0], *b1 = h->buf[1];
+            int cur = h->cur, nn = n < lbm::PERSIST_MAX_STEPS ? n : lbm::PERSIST_MAX_STEPS;
+            static_assert(lbm::BARRIER_START == 0xFFFFFFFFu, "the byte memset below writes BARRIER_START");
+            CUDA_TRY(cudaMemsetAsync(h->d_counter, 0xFF, sizeof(unsigned), st));
+            void *args[] = {&a, &b0, &b1, &cur, &nn, &h->d_counter};
+            le = cudaLaunchCooperativeKernel(fn, dim3(h->persist_blocks), dim3(h->persist_tb), args, 0, st);
+            launched = le == cudaSuccess;
+            if (launched) {
+                h->launches++;
+                h->wrap_ok[0] = h->wrap_ok[1] = false;
+                if (nn % 2) h->cur ^= 1;
+                h->steps += nn;
+                n -= nn;
+            }
         }
-        // the grid is not co-resident after all (a shared or partitioned GPU): launched steps from now on, outside capture
+        if (launched) return LBM_OK;
         cudaGetLastError();
+        // Only "the grid is not co-resident after all" (a shared or partitioned GPU) turns the persistent path off for
+        // good: launched steps from now on.  Anything else (a bad stream, a broken capture) is the caller's to see.
+        if (le != cudaErrorCooperativeLaunchTooLarge && le != cudaErrorLaunchOutOfResources)
+            return fail(LBM_ERR_CUDA, "lbm_step: cooperative launch of the persistent kernel: %s", cudaGetErrorString(le));
         h->persist_blocks = 0;
         if (cap != cudaStreamCaptureStatusNone && n % 2)
             return fail(LBM_ERR_INVALID, "lbm_step: %d launched steps cannot be captured (odd number of swaps)", n);

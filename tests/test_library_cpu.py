@@ -158,3 +158,10 @@ def test_two_step_kernel_releases_buffers_only_after_consuming_them(lib):
         i += 1
     assert gathers >= 2, f"expected the producers' and the consumers' gathers, found {gathers}"
     assert any(o.startswith("FENCE.VIEW.ASYNC") for o in ops), "the stage reads are not fenced into the async proxy"
+
+
+def test_slab_buffer_bytes_refuses_what_create_slab_refuses(lib):
+    """the size query and lbm_create_slab agree on the smallest slab (6 own rows)."""
+    for nz in (3, 4, 5):
+        assert lib.lbm_slab_buffer_bytes(64, 128, 10, nz) == 0
+    assert lib.lbm_slab_buffer_bytes(64, 128, 10, 6) > 0
