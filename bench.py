@@ -32,10 +32,26 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the committed `ncu --set full`
 # captures under profiles/ -- NOT measured in this run: reported with its source file, and only when this run's launch
 # (workload, steps per launch, strip width, rows per chunk) is the one that was captured; null otherwise.
+# The key ends with the git blob hash of the kernel's source file at capture time: an edit to the kernel nulls the figure
+# until the capture is redone.
 NCU_TRAFFIC = {
-    ("rt_single_4096x8192", 1, None, None): (19.839e9, "profiles/r2_step_kernels_full.md"),
-    ("rt_single_4096x8192", 2, 56, 410): (20.203e9, "profiles/r2_step2s_kernel_full.md"),
+    ("rt_single_4096x8192", 1, None, None, "lbm_step.cuh", "f0747db8b6c7e93d7466d3f6ff90472b7d15c26c"): (19.839e9, "profiles/r2_step_kernels_full.md"),
+    ("rt_single_4096x8192", 2, 56, 410, "lbm_step2s.cuh", "c0d3233db4eb1e5fd65842c20e8c94a986c75cb7"): (20.203e9, "profiles/r2_step2s_kernel_full.md"),
 }
+
+
+def git_blob_hash(path: str) -> str:
+    """What `git hash-object` prints for the file (sha1 of "blob <size>\\0" + contents)."""
+    import hashlib
+    data = open(path, "rb").read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def ncu_traffic(workload, spl, strip_w, zchunk):
+    src = "lbm_step2s.cuh" if spl > 1 else "lbm_step.cuh"
+    blob = git_blob_hash(os.path.join(ROOT, "paper_1405_1253_b200", "csrc", src))
+    key = (workload, spl, strip_w if spl > 1 else None, zchunk if spl > 1 else None, src, blob)
+    return NCU_TRAFFIC.get(key, (None, None))
 
 
 def measured_peak():
@@ -77,16 +93,22 @@ class ClockSampler(threading.Thread):
                 self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
             except Exception:
                 pass
-            time.sleep(0.02)
+            time.sleep(0.002)
+
+    def mark(self):
+        """The timed region starts here: only later samples (and their throttle reasons) are reported."""
+        self._first = len(self.samples)
+        self.mask = 0
 
     def finish(self) -> dict:
         self._halt.set()
         if self.is_alive():
             self.join()
-        if not self.samples:
+        mine = self.samples[getattr(self, "_first", 0):]
+        if not mine:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
-        s = sorted(self.samples)
-        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "samples": len(s),
+        s = sorted(mine)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "samples": len(s), "period_ms": 2,
                 "reasons": [n for b, n in self.REASONS.items() if self.mask & b]}
 
 
@@ -189,6 +211,36 @@ def whole_job_mlups(sites_per_rank: int, steps: int, world: int, seconds_max: fl
     return world * sites_per_rank * steps / seconds_max / 1e6
 
 
+def a6_kernel_times(lat, cfg, stream, torch, reps: int = 5):
+    """Row a6 kernels at this workload, timed with CUDA events outside the driver's timed region: moments_kernel (reads
+    the 37 populations, writes rho, u_x, u_z, T: 328 B per site) and the one-pass diagnostics
+    (row_diagnostics_kernel<false> + final_diagnostics_kernel: 296 B per site read; <true> re-reads each row for the
+    squared deviations, from L2).  Peak: the measured copy bandwidth.  Traffic: profiles/r3_a6_kernels.md."""
+    peak, peak_kind = measured_peak()
+    sites = cfg.Lx * cfg.Lz
+    fields = [torch.empty((cfg.Lz, cfg.Lx), dtype=torch.float64, device="cuda") for _ in range(4)]
+
+    def timed(fn):
+        fn(); torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / reps
+
+    out = {"peak": peak, "peak_kind": peak_kind, "unit": "GB/s", "bound": "hbm"}
+    for name, nbytes, fn in (
+            ("moments_kernel", 328, lambda: lat.moments(*fields)),
+            ("row_diagnostics_kernel<false>+final", 296, lambda: lat.diagnostics(cfg.T_d, cfg.T_m, cfg.T_u, profiles=False)),
+            ("row_diagnostics_kernel<true>+final", 296, lambda: lat.diagnostics(cfg.T_d, cfg.T_m, cfg.T_u, profiles=True, rms=True))):
+        t = timed(fn)
+        out[name] = {"bytes_per_site": nbytes, "ms": t * 1e3, "achieved": nbytes * sites / t / 1e9,
+                     "frac": nbytes * sites / t / 1e9 / peak}
+    out["note"] = "the diagnostics calls copy their results to the host and synchronise: their time includes that"
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -214,7 +266,7 @@ def run_ours(args):
         cfg = si.scaled(cfg, args.lx, args.lz)
     sites = cfg.Lx * cfg.Lz
     stream = torch.cuda.current_stream()
-    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, wall_kind=args.wall_kind, T_wall=(cfg.T_d, cfg.T_u))
     if args.variant is not None:
         lat.set_variant(args.variant)
     if args.zchunk:
@@ -229,11 +281,12 @@ def run_ours(args):
             torch.cuda.synchronize()
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps + one widths call
+    sampler = ClockSampler(local)                            # running before the warm-up, so that it is sampling at
+    sampler.start()                                          # full rate when the (short) timed region begins
     lat.step(args.warmup)
     lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
+    sampler.mark()
     l0 = lat.kernel_launches
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     ev[0].record(stream)
@@ -271,11 +324,9 @@ def run_ours(args):
                      "reasons": c2.get("reasons")}
 
     # ---- end to end through lbm_run_host: pinned host fields in, K steps, host fields out
-    g = cfg.g
-    rho, ux, uz, T = lat.moments()
-    host_in = [x.cpu().pin_memory() for x in (rho, ux, uz - 0.5 * g, T - 0.125 * g * g)]  # kinetic fields
+    a6 = a6_kernel_times(lat, cfg, stream, torch) if rank == 0 else None
+    host_in = [x.cpu().pin_memory() for x in lat.kinetic_moments()]     # what lbm_run_host takes (lbm_kinetic_moments)
     host_out = tuple(torch.empty_like(x).pin_memory() for x in host_in)
-    del rho, ux, uz, T
     fp64_peak = max(pkg.fp64_peak() for _ in range(2))                  # TFLOP/s, DFMA chains on all SMs (clock under load)
     e2e_steps = args.e2e_steps or args.steps
     lat.run_host(*host_in, n=min(3, e2e_steps), outs=host_out)          # warm-up (allocates staging)
@@ -306,6 +357,10 @@ def run_ours(args):
     n_step_kernels = (args.steps // 2 + args.steps % 2) if fused else args.steps
     if args.variant in (1, 2):
         n_step_kernels = args.steps
+    # tiny lattices: ONE cooperative launch of step_persistent_kernel runs all K steps (the handle counted one launch)
+    persistent = not fused and args.variant in (None, 0) and step_launches == 1 and args.steps > 1
+    if persistent:
+        n_step_kernels = 1
     spl = args.steps / max(n_step_kernels, 1)
     launch_ms = t_steps / max(n_step_kernels, 1) * 1e3
     alg_bytes = BYTES_PER_SITE * sites * spl
@@ -315,12 +370,13 @@ def run_ours(args):
     compulsory = BYTES_PER_SITE * sites
     own_gbs = compulsory / (launch_ms * 1e-3) / 1e9
     whole = abs(spl - round(spl)) < 1e-9
-    key = (cfg.name, int(round(spl)), strip_w if spl > 1.5 else None, zchunk if spl > 1.5 else None)
-    traffic, traffic_source = NCU_TRAFFIC.get(key, (None, None)) if whole else (None, None)
+    traffic, traffic_source = ncu_traffic(cfg.name, int(round(spl)), strip_w, zchunk) if whole and args.wall_kind == 0 else (None, None)
     rate = sites * spl / (launch_ms * 1e-3)                        # site-steps per second of the kernel
     roofline = {"bound": "hbm",
-                "kernel": "step2s_kernel (two fused propagate+bc+collide steps per launch)" if spl > 1.5
+                "kernel": "step_persistent_kernel (all K steps in one cooperative launch, grid barrier between steps; L2-resident)" if persistent
+                else "step2s_kernel (two fused propagate+bc+collide steps per launch)" if spl > 1.5
                 else "step_kernel_site (fused propagate+bc+collide)",
+                "frac_of_compulsory_dram": own_gbs / peak,
                 "achieved": achieved, "peak": peak,
                 "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
                 "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
@@ -366,10 +422,10 @@ def run_ours(args):
         "config": {"workload": cfg.name, "Lx": cfg.Lx, "Lz": cfg.Lz, "tau": cfg.tau, "g": cfg.g,
                    "parallelism": "replicas only" if world > 1 else "single GPU, whole lattice resident",
                    "l2": "inputs larger than L2 (2 x 37 planes, %.1f GB)" % (2 * 37 * 8 * sites / 1e9),
-                   "variant": args.variant, "widths_calls_in_timed_region": 1,
+                   "variant": args.variant, "wall_kind": args.wall_kind, "widths_calls_in_timed_region": 1,
                    "L_u": widths[0], "L_d": widths[1]},
         "sustained": sustained,
-        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "roofline": roofline, "roofline_a6": a6, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
     }))
     if world > 1:
         dist.destroy_process_group()
@@ -575,6 +631,7 @@ def main():
     ap.add_argument("--lx", type=int, default=0)
     ap.add_argument("--lz", type=int, default=0)
     ap.add_argument("--variant", type=int, default=None, help="step-kernel variant (default: library default)")
+    ap.add_argument("--wall-kind", type=int, default=0, choices=[0, 1], help="0 bounce-back walls (default), 1 isothermal no-slip walls")
     ap.add_argument("--zchunk", type=int, default=0, help="rows per block of the two-step kernel (multiple of 3)")
     ap.add_argument("--e2e-steps", type=int, default=0)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle time for cpu_baseline")

@@ -166,6 +166,12 @@ int lbm_step(lbm_t *h, int n, void *stream);
  * Asynchronous. */
 int lbm_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *stream);
 
+/* The KINETIC moments rho, u, T of eq. 7 of the stored state, without the half-force shift of
+ * PAPER.md:94 that lbm_moments applies: exactly the fields lbm_init_equilibrium and lbm_run_host take, so a state
+ * can be handed from one to the other without arithmetic on the caller's side.  DEVICE arrays [Lz][Lx], any may be
+ * NULL (not all).  Asynchronous. */
+int lbm_kinetic_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *stream);
+
 /* Mixing widths of eq. 12 from the x-averaged T^(H), in sites, with the
  * tent map of eq. 9 (zero outside [0,1]).  L_u, L_d: HOST doubles; Tbar: HOST array [Lz] or NULL.
  * Synchronises `stream`. */

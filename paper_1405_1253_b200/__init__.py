@@ -193,6 +193,15 @@ class Lattice:
         return rho, ux, uz, T
 
     @_on_device
+    def kinetic_moments(self, stream=None):
+        """(rho, ux, uz, T) of eq. 7 without the half-force shift (lbm_kinetic_moments): the inputs of
+        init_equilibrium / run_host.  New device tensors [Lz][Lx]."""
+        import torch
+        out = tuple(torch.empty((self.Lz, self.Lx), dtype=torch.float64, device=self.device) for _ in range(4))
+        binding.check(self._lib.lbm_kinetic_moments(self._h, *[_dptr(x) for x in out], _stream_ptr(stream, self.device)))
+        return out
+
+    @_on_device
     def mixing_widths(self, T_d, T_m, T_u, want_tbar=True, stream=None):
         import numpy as np
         lu, ld = C.c_double(), C.c_double()

@@ -22,7 +22,7 @@ SYMBOLS = [
     "lbm_layout", "lbm_kernel_launches", "lbm_fp64_peak", "lbm_set_variant", "lbm_set_zchunk", "lbm_get_plan", "lbm_tables", "lbm_last_error",
     "lbm_diagnostics", "lbm_rt_scales", "lbm_slab_buffer_bytes", "lbm_create_slab", "lbm_slab_info", "lbm_slab_pack",
     "lbm_slab_unpack", "lbm_slab_step", "lbm_get_window", "lbm_slab_pack2", "lbm_slab_unpack2", "lbm_slab_step2",
-    "lbm_diagnostics_noalloc",
+    "lbm_diagnostics_noalloc", "lbm_kinetic_moments",
 ]
 
 
@@ -66,6 +66,7 @@ def load():
         getattr(L, name).argtypes = [vp, vp, vp]
     L.lbm_step.argtypes = [vp, C.c_int, vp]
     L.lbm_moments.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.lbm_kinetic_moments.argtypes = [vp, vp, vp, vp, vp, vp]
     L.lbm_mixing_widths.argtypes = [vp, C.c_double, C.c_double, C.c_double, dp, dp, vp, vp]
     L.lbm_profiles.argtypes = [vp, vp, vp, vp, vp, vp]
     L.lbm_growth_rate.argtypes = [C.c_int, vp, vp, C.c_double, C.c_double, vp]

@@ -838,6 +838,17 @@ int lbm_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *
     return LBM_OK;
 }
 
+// eq. 7 as it stands (moments_kernel with no gravity shift): the inputs lbm_init_equilibrium / lbm_run_host take
+int lbm_kinetic_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *stream)
+{
+    NEED(h);
+    if (!rho && !ux && !uz && !T) return fail(LBM_ERR_INVALID, "lbm_kinetic_moments: all four outputs are null");
+    lbm::moments_kernel<<<own_grid(h, lbm::AUX_TX), lbm::AUX_TX, 0, (cudaStream_t)stream>>>(
+        h->buf[h->cur], h->layout(), 0.0, rho, ux, uz, T);
+    LAUNCHED(h);
+    return LBM_OK;
+}
+
 // one pass over the lattice + one small block; results stay in the handle's scratch
 static int run_diagnostics(lbm_t *h, bool want_rms, double T_d, double T_m, double T_u, cudaStream_t st)
 {

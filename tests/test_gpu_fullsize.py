@@ -29,7 +29,7 @@ def _window(dense, r0, r1, cols):
     return dense[:, r0:r1][:, :, cols].contiguous().cpu().numpy()
 
 
-def _check_windows(orc, before, after, Lx, Lz, tau, g, tol, plan=None):
+def _check_windows(orc, before, after, Lx, Lz, tau, g, tol, plan=None, walls=None):
     """before/after: dense device populations [37][Lz][Lx] at step 0 and step NSTEPS.  With `plan` = (fused, strip
     width w, rows per chunk ZC) of the launch, extra windows straddle a chunk boundary (rows around c ZC, where one
     block hands over to the next: ring wrap, warm-up rows) and a strip boundary (columns around s w)."""
@@ -58,12 +58,110 @@ def _check_windows(orc, before, after, Lx, Lz, tau, g, tol, plan=None):
         cols = (torch.arange(c0, c0 + W, device=before.device) % Lx)
         w0 = _window(before, r0, r0 + W, cols)
         w1 = _window(after, r0, r0 + W, cols)
-        ref = orc.step(w0, tau, g, nsteps=NSTEPS, periodic_z=(kind == "bulk"))
+        if walls is not None and kind != "bulk":   # wall_kind 1: `walls` = (T_bottom, T_top); bulk rows do not see the wall rule
+            ref = orc.step(w0, tau, g, nsteps=NSTEPS, wall_kind=1, T_bot=walls[0], T_top=walls[1])
+        else:
+            ref = orc.step(w0, tau, g, nsteps=NSTEPS, periodic_z=(kind == "bulk"))
         rows = slice(0, W - M) if kind == "bottom" else slice(M, W) if kind == "top" else slice(M, W - M)
         a, b = w1[:, rows, M:W - M], ref[:, rows, M:W - M]
         worst = max(worst, float(np.max(np.abs(a - b) / np.abs(b))))
     assert worst < tol, worst
     return worst
+
+
+def _check_row_slabs_after_n_steps(orc, lat, cfg, n, centres, tol, walls=None, h=24):
+    """The north_star criterion at full size: `lat` (initialised, at step 0) is stepped n times; for each (kind, row)
+    of `centres` the oracle steps a full-width slab (exact periodic x) of h rows plus 3n rows of halo -- the domain of
+    dependence of a row after n steps -- and the h rows are compared population by population.  Bulk slabs are closed
+    periodically in z (the wrong closure stays within the halo); wall slabs have the real wall on one side."""
+    halo = 3 * n
+    spans = []
+    for kind, centre in centres:
+        if kind == "bulk":
+            spans.append((centre - h // 2 - halo, centre + h // 2 + halo, slice(halo, halo + h)))
+        elif kind == "bottom":
+            spans.append((0, h + halo, slice(0, h)))
+        else:
+            spans.append((cfg.Lz - h - halo, cfg.Lz, slice(halo, halo + h)))
+    assert all(0 <= r0 and r1 <= cfg.Lz for r0, r1, _ in spans), spans
+    before = [lat.get_window(r0, r1 - r0, 0, cfg.Lx).cpu().numpy() for r0, r1, _ in spans]
+    lat.step(n)
+    worst = 0.0
+    for (kind, _), (r0, r1, rows), w0 in zip(centres, spans, before):
+        w1 = lat.get_window(r0, r1 - r0, 0, cfg.Lx).cpu().numpy()
+        if walls is not None and kind != "bulk":
+            ref = orc.step(w0, cfg.tau, cfg.g, nsteps=n, wall_kind=1, T_bot=walls[0], T_top=walls[1])
+        else:
+            ref = orc.step(w0, cfg.tau, cfg.g, nsteps=n, periodic_z=(kind == "bulk"))
+        worst = max(worst, float(np.max(np.abs(w1[:, rows] - ref[:, rows]) / np.abs(ref[:, rows]))))
+        del w1, ref
+    assert worst < tol, worst
+    return worst
+
+
+def test_config4_100_steps_slabs_against_oracle(pkg, orc):
+    """the headline lattice (BASELINE.json configs[3], 4096x8192) in the launch bench.py times, after
+    100 steps -- the north_star criterion, 1e-11 per population -- on full-width row slabs at the interface, at both
+    walls and across a chunk boundary of the launch plan; lattice totals to 1e-12."""
+    cfg = si.rt_config(4)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g)
+    fused, w, zc = lat.plan()
+    assert fused and zc < cfg.Lz
+    nchunks = (cfg.Lz + zc - 1) // zc
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    t0 = lat.totals()
+    centres = [("bulk", cfg.Lz // 2), ("bottom", 0), ("top", cfg.Lz), ("bulk", (nchunks // 4) * zc)]
+    _check_row_slabs_after_n_steps(orc, lat, cfg, 100, centres, 1e-11)
+    t1 = lat.totals()
+    assert abs(t1[0] / t0[0] - 1) < 1e-12                    # mass
+    lat.close()
+
+
+def test_isothermal_walls_at_size_with_the_automatic_plan(pkg, orc):
+    """wall_kind 1 runs its own instances of the step kernels.  2048x4096 (config 3), automatic plan,
+    100 steps: both wall slabs against the oracle's isothermal-wall step and the lower interface, 1e-11.
+    4096x8192 (config 4): 7-step windows on both walls, the seam, strip and chunk boundaries, 1e-13."""
+    cfg = si.rt_config(3)
+    walls = (cfg.T_d, cfg.T_u)
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, wall_kind=1, T_wall=walls)
+    assert lat.plan()[0]
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    _check_row_slabs_after_n_steps(orc, lat, cfg, 100, [("bottom", 0), ("top", cfg.Lz), ("bulk", int(cfg.Lz / 2 - cfg.delta / 2))],
+                                   1e-11, walls=walls)
+    lat.close()
+    cfg = si.rt_config(4)
+    walls = (cfg.T_d + 0.01, cfg.T_u - 0.01)                 # walls that differ from the fluid next to them
+    lat = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, wall_kind=1, T_wall=walls)
+    plan = lat.plan()
+    assert plan[0] and plan[2] < cfg.Lz
+    lat.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    before = lat.get_populations()
+    lat.step(NSTEPS)
+    after = lat.get_populations()
+    _check_windows(orc, before, after, cfg.Lx, cfg.Lz, cfg.tau, cfg.g, 1e-13, plan, walls=walls)
+    lat.close()
+
+
+def test_two_slabs_of_config3_isothermal_walls_fused_path_equal_the_whole_lattice(pkg):
+    """config 3 with wall_kind 1 as two z-slabs stepped with the two-step kernel (pack2 / unpack2 /
+    step2), 50 steps, against the whole lattice with the automatic plan: bit-identical."""
+    import torch
+    from test_gpu_variants import _run_slabs_fused
+    cfg = si.rt_config(3)
+    kw = dict(wall_kind=1, T_wall=(cfg.T_d, cfg.T_u))
+    whole = pkg.Lattice(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, **kw)
+    assert whole.plan()[0]
+    whole.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    whole.step(50)
+    ref = whole.get_populations()
+    whole.close()
+    slabs = [pkg.Slab(cfg.Lx, cfg.Lz, z0, nz, cfg.tau, cfg.g, **kw) for z0, nz in ((0, 2048), (2048, 2048))]
+    for s in slabs:
+        s.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
+    _run_slabs_fused(pkg, slabs, 25)
+    for s, rows in zip(slabs, (slice(0, 2048), slice(2048, 4096))):
+        assert torch.equal(s.get_populations(), ref[:, rows])
+        s.close()
 
 
 def test_config4_fullsize_sampled_windows_and_conservation(pkg, orc):

@@ -143,6 +143,17 @@ def test_init_equilibrium_moments_and_widths(pkg, orc):
     mo = orc.moments(ref, g)
     assert np.max(np.abs(m[0] - mo[0])) < 1e-13 and np.max(np.abs(m[3] - mo[3])) < 1e-13
     assert np.max(np.abs(m[1] - mo[1])) < 1e-14 and np.max(np.abs(m[2] - mo[2])) < 1e-14
+    # kinetic moments (eq. 7, no half-force shift) = the oracle's moments at g = 0; fed back through
+    # init_equilibrium they reproduce themselves (what bench.py's end-to-end leg relies on)
+    km = lat.kinetic_moments()
+    ko = orc.moments(ref, 0.0)
+    for a, b in zip(km, ko):
+        assert np.max(np.abs(a.cpu().numpy() - b)) < 1e-13
+    again = pkg.Lattice(Lx, Lz, 0.8, g)
+    again.init_equilibrium(*km)
+    for a, b in zip(again.kinetic_moments(), km):
+        assert float((a - b).abs().max()) < 1e-13
+    again.close()
     lu, ld, tbar = lat.mixing_widths(1.05, 1.0, 0.95)
     olu, old, otbar = orc.mixing_widths(ref, g, 1.05, 1.0, 0.95)
     assert np.max(np.abs(tbar - otbar)) < 1e-13 and abs(lu - olu) < 1e-10 and abs(ld - old) < 1e-10
