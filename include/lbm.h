@@ -259,7 +259,9 @@ int lbm_set_zchunk(lbm_t *h, int rows);  /* rows per block of the two-step kerne
 /* The launch plan lbm_step uses for this lattice with the current variant / zchunk settings (HOST outputs, any may
  * be NULL): *fused = 1 if a launch advances two time steps (two-step kernel), 0 if one; *strip_width = columns per
  * block of the two-step kernel (strip s covers columns [s w, (s+1) w)); *zchunk = rows per block (chunk c covers
- * rows [c ZC, (c+1) ZC)).  Automatic choice: DESIGN.md section 6 (whole waves of blocks, few chunks). */
+ * rows [c ZC, (c+1) ZC)).  Automatic choice: DESIGN.md section 6 (whole waves of blocks, few chunks).  With
+ * wall_kind 1 and an automatic plan of several chunks the chunks on an isothermal wall are 14 rows shorter (their wall
+ * adjustments cost about that much): chunk c > 0 then starts at row c ZC - 14, the last chunk ends at Lz. */
 int lbm_get_plan(lbm_t *h, int *fused, int *strip_width, int *zchunk);
 /* D2Q37 tables as the library uses them (host outputs, any may be NULL): e_x[37], e_z[37], w[37], r. */
 int lbm_tables(int *ex, int *ez, double *w, double *r);

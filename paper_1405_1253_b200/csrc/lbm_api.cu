@@ -4,6 +4,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -114,6 +115,7 @@ bool encode_step2s_maps(const double *ubuf, int Lx, int Lz, int pitch, long long
 struct lbm_plan {
     bool valid, fused;
     int w, strips, ZC, chunks;
+    int trim;       // wall_kind 1: rows the chunks next to an isothermal wall are shorter by (chunk boundaries shift down by it)
 };
 
 struct lbm_handle {
@@ -187,6 +189,7 @@ lbm::StepArgs step_args(const lbm_t *h)
     a.Tw_hi = h->T_wall_hi - 0.125 * h->g * h->g;
     a.wrap_store = 0;
     a.w = 0;
+    a.ztrim = 0;
     a.zbase = h->glo; a.zend = h->glo + h->nz;
     lbm::fill_offsets(a);
     return a;
@@ -207,6 +210,8 @@ const lbm_plan &make_plan(lbm_t *h)
     lbm_plan &p = h->plan;
     p = lbm_plan{};
     const int Lx = h->Lx, Lz = h->nz, sms = h->sm_count > 0 ? h->sm_count : 148;   // rows to update: a slab's own
+    const bool iso_lo = h->wall_kind == 1 && h->wall_lo(), iso_hi = h->wall_kind == 1 && h->wall_hi();
+    constexpr int ISO_TRIM = 14;
     const int ns_min = (Lx + S2::TX - 1) / S2::TX;
     double best = 1e300;
     for (int ns = ns_min; ns <= ns_min + ns_min / 4 + 1; ++ns) {
@@ -216,18 +221,28 @@ const lbm_plan &make_plan(lbm_t *h)
         if (w < 8) w = 8;
         const int strips = (Lx + w - 1) / w;
         for (int chunks = 1; chunks <= (Lz + 15) / 16; ++chunks) {
-            int ZC = (Lz + chunks - 1) / chunks;
+            // wall_kind 1: a block on an isothermal wall spends four of its passes on the wall adjustment of rows
+            // 0..2 / Lz-3..Lz-1 in both steps (two more equilibrium evaluations per site, ~2.9 us per such pass against
+            // ~1.7 us: +11 us measured at 512x1024, profiles/r3_wall_kind1.md), and a launch waits for its slowest
+            // block: those chunks are ISO_TRIM rows shorter, the others share the rows.
+            int tlo = iso_lo ? ISO_TRIM : 0, thi = iso_hi ? ISO_TRIM : 0;
+            int ZC = (Lz + tlo + thi + chunks - 1) / chunks;
             ZC = (ZC + 1) / 2 * 2;                            // whole passes of R = 2 rows
+            if (chunks == 1 || ZC < 4 * ISO_TRIM) {           // nothing to balance against / chunks too short to trim
+                tlo = thi = 0;
+                ZC = ((Lz + chunks - 1) / chunks + 1) / 2 * 2;
+            }
             if (ZC < 6) ZC = 6;
-            const int nch = (Lz + ZC - 1) / ZC;
+            const int nch = (Lz + tlo + ZC - 1) / ZC;
             const long long waves = ((long long)strips * nch + sms - 1) / sms;
             // x (1 + ZC / 16000): blocks that march for thousands of rows drift apart, and the columns two neighbouring
             // strips both load stop meeting in L2 (4096x8192 in one wave of 4096-row chunks: -6 %)
             const double cost = ((double)waves + 0.15) * (ZC + 6 + 10) * (1.0 + ZC / 16000.0);
-            if (cost < best - 1e-9) { best = cost; p.w = w; p.strips = strips; p.ZC = ZC; p.chunks = nch; }
+            if (cost < best - 1e-9) { best = cost; p.w = w; p.strips = strips; p.ZC = ZC; p.chunks = nch; p.trim = tlo; }
         }
     }
     if (h->zchunk > 0) {                                      // rows per block forced (tests, experiments)
+        p.trim = 0;
         p.ZC = h->zchunk;
         p.chunks = (Lz + p.ZC - 1) / p.ZC;
         best = ((double)(((long long)p.strips * p.chunks + sms - 1) / sms) + 0.15) * (p.ZC + 16) * (1.0 + p.ZC / 16000.0);
@@ -292,7 +307,17 @@ int one_step_rows(lbm_t *h, lbm::StepArgs &a, int k0, int k1, cudaStream_t st)
 {
     a.src = h->buf[h->cur];
     a.dst = h->inplace ? h->buf[h->cur] : h->buf[h->cur ^ 1];
-    return h->wall_kind == 1 ? launch_one_step<true>(h, a, k0, k1, st) : launch_one_step<false>(h, a, k0, k1, st);
+    if (h->wall_kind != 1) return launch_one_step<false>(h, a, k0, k1, st);
+    // wall_kind 1: the instance with the wall adjustment (twice the code, a dozen spilled registers) is needed by the
+    // three rows next to an isothermal wall only.  Where two extra launches cost nothing (large lattices) those rows
+    // get launches of their own and the rest runs the plain instance; rows of a launch are independent of each other.
+    if ((long long)h->Lx * h->Lz < (1LL << 20)) return launch_one_step<true>(h, a, k0, k1, st);
+    const int lo = a.iso_lo ? std::min(k1, std::max(k0, 3)) : k0;
+    const int hi = a.iso_hi ? std::max(lo, std::min(k1, h->Lz - 3)) : k1;
+    int rc = launch_one_step<true>(h, a, k0, lo, st);
+    if (!rc) rc = launch_one_step<false>(h, a, lo, hi, st);
+    if (!rc) rc = launch_one_step<true>(h, a, hi, k1, st);
+    return rc;
 }
 
 // a5: after a step the other copy is current (two copies) or the layout has alternated (one copy)
@@ -312,6 +337,7 @@ int launch_two_step(lbm_t *h, lbm::StepArgs &a, const lbm_plan &plan, cudaStream
     using S2 = lbm::Step2sWide;
     dim3 grid(plan.strips, plan.chunks);
     a.w = plan.w;
+    a.ztrim = plan.trim;
     // the consumers' spare lanes of the two seam strips keep the wrap columns of the destination current, if the
     // seam columns [0, XW) and [Lx - XW, Lx) each lie within one strip and that strip has XW lanes to spare (2 XW
     // if it is the only strip); else the columns are refreshed before every launch

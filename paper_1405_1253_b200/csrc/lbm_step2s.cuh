@@ -368,9 +368,11 @@ __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_cons
     __shared__ unsigned long long bars[2 * S::NRB + 2 * S::NST];
     const int tid = threadIdx.x;
     const int w = a.w;                                   // strips of w <= TX columns (w even: TMA boxes start on 16 bytes)
-    const int x0 = blockIdx.x * w, z0 = a.zbase + blockIdx.y * ZC;   // a z-slab updates its own rows; its ghost rows are sources only
+    // a z-slab updates its own rows; its ghost rows are sources only.  ztrim (wall_kind 1): the chunk on an isothermal
+    // wall is that many rows shorter, which is what its wall adjustments cost (lbm_api.cu make_plan)
+    const int x0 = blockIdx.x * w, z0 = a.zbase + blockIdx.y * ZC - (blockIdx.y ? a.ztrim : 0);
     const int ncols = min(w, a.Lx - x0);                // output columns of this strip
-    const int zend = min(a.zend, z0 + ZC);              // output rows [z0, zend)
+    const int zend = min(a.zend, a.zbase + ((int)blockIdx.y + 1) * ZC - a.ztrim);   // output rows [z0, zend)
     const int rlast = min(a.Lz, zend + 3);              // intermediate rows [max(0, z0-3), rlast)
     const int NP = (zend - z0 + S::R - 1) / S::R;       // consumer passes
     const unsigned bar_full = (unsigned)__cvta_generic_to_shared(&bars[0]);     // [NRB] ring rows written (producers -> consumers)
@@ -384,12 +386,21 @@ __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_cons
     }
     __syncthreads();
     double *stage = smem2s + S::RING_DOUBLES;
-    if (tid < S::NAT)
-        step2s_producer<S, ISO>(a, smem2s, stage, bar_full, tid, x0, z0, ncols, rlast, NP);
-    else if (tid < S::NAT + S::NBT)
-        step2s_consumer<S, ISO>(a, smem2s, bar_full, bar_empty, tid - S::NAT, x0, z0, ncols, zend);
-    else
+    // wall_kind 1 (ISO): only the chunks that hold one of the three rows next to an isothermal wall -- as intermediate
+    // rows [z0-3, zend+3) or as output rows -- run the roles with the wall adjustment; every other block of the launch
+    // runs the plain roles (separate non-inlined functions, so the larger code and the spills of the wall roles cost
+    // the bulk of the lattice nothing: "computational impact is fully negligible").
+    bool wall_chunk = false;
+    if constexpr (ISO) wall_chunk = (a.iso_lo && z0 < 6) || (a.iso_hi && zend + 6 > a.Lz);
+    if (tid < S::NAT) {
+        if (wall_chunk) step2s_producer<S, true>(a, smem2s, stage, bar_full, tid, x0, z0, ncols, rlast, NP);
+        else step2s_producer<S, false>(a, smem2s, stage, bar_full, tid, x0, z0, ncols, rlast, NP);
+    } else if (tid < S::NAT + S::NBT) {
+        if (wall_chunk) step2s_consumer<S, true>(a, smem2s, bar_full, bar_empty, tid - S::NAT, x0, z0, ncols, zend);
+        else step2s_consumer<S, false>(a, smem2s, bar_full, bar_empty, tid - S::NAT, x0, z0, ncols, zend);
+    } else {
         step2s_loader<S>(&maps, stage, bar_sfull, bar_sempty, tid - S::NAT - S::NBT, x0, z0, NP);
+    }
 }
 
 }  // namespace lbm
