@@ -447,13 +447,20 @@ def run_slabs(args):
     rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
     if world < 2:
         raise SystemExit("bench.py --slabs needs torchrun with N > 1 ranks")
+    # --backend gloo: the ranks may share GPUs (messages staged through pinned host memory): runs the whole schedule on
+    # a one-GPU box; the number it prints is a smoke value, not a scaling measurement
+    local = local % torch.cuda.device_count()
     torch.cuda.set_device(local)
-    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        dist.init_process_group(args.backend)
+    red_dev = "cuda" if args.backend == "nccl" else "cpu"
     if rank == 0:
         entry.build()
     dist.barrier()
     cfg = si.rt_config(args.config)
-    ring = SlabRing(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, rank, world)
+    ring = SlabRing(cfg.Lx, cfg.Lz, cfg.tau, cfg.g, rank, world, wall_kind=args.wall_kind, T_wall=(cfg.T_d, cfg.T_u))
     ring.slab.init_rt(si.DEFAULT_SEED, **cfg.rt_args())
     stream = torch.cuda.current_stream()
 
@@ -468,9 +475,9 @@ def run_slabs(args):
     e0.record(stream); ring.step(args.steps); e1.record(stream)
     barrier()
     clocks = sampler.finish()
-    t = reduce_max([e0.elapsed_time(e1) * 1e-3], world, "cuda")[0]
+    t = reduce_max([e0.elapsed_time(e1) * 1e-3], world, red_dev)[0]
     part = ring.slab.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u, want_tbar=False)
-    w = torch.tensor([part[0], part[1]], dtype=torch.float64, device="cuda")
+    w = torch.tensor([part[0], part[1]], dtype=torch.float64, device=red_dev)
     dist.all_reduce(w)                                           # the widths of eq. 12 are sums over rows
     launches = ring.slab.kernel_launches - l0
     if rank == 0:
@@ -481,7 +488,9 @@ def run_slabs(args):
             "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "Lx": cfg.Lx, "Lz": cfg.Lz, "tau": cfg.tau, "g": cfg.g,
                        "parallelism": f"{world} z-slabs; pairs of steps with the two-step kernel (6 whole ghost rows per open "
-                                      "side and pair), an odd step with the one-step kernel (26 population-rows, interior first)",
+                                      "side and pair), an odd step with the one-step kernel (26 population-rows); interior rows first, "
+                                      "the exchange behind them",
+                       "backend": args.backend, "wall_kind": args.wall_kind,
                        "message2_bytes": 6 * 37 * (cfg.Lx + 16) * 8, "message_bytes": 26 * cfg.Lx * 8,
                        "L_u": float(w[0]), "L_d": float(w[1])},
             "gpu_launches": launches, "clocks": clocks}))
@@ -547,19 +556,25 @@ def run_slabs_local(args):
 
     mlups_slabs = timed(step_slabs)
 
-    # the same slabs with the two-step kernel: 6 whole ghost rows per open side and pair of steps, no interior/edge split
+    # the same slabs with the two-step kernel: 6 whole ghost rows per open side and pair of steps, interior rows first
     up2, dn2, below2, above2 = ([s.new_message(True) for s in slabs] for _ in range(4))
 
     def step_slabs_fused(n):
         for _ in range(n // 2):
+            xs.wait_stream(main)
             for i, s in enumerate(slabs):
-                if s.open_above: s.pack2(1, up2[i])
-                if s.open_below: s.pack2(0, dn2[i])
-            for i, s in enumerate(slabs):
-                if s.open_below: below2[i].copy_(up2[i - 1], non_blocking=True); s.unpack2(0, below2[i])
-                if s.open_above: above2[i].copy_(dn2[i + 1], non_blocking=True); s.unpack2(1, above2[i])
+                if s.open_above: s.pack2(1, up2[i], stream=xs)
+                if s.open_below: s.pack2(0, dn2[i], stream=xs)
+            main.wait_stream(xs)
             for s in slabs:
-                s.step2()
+                s.step2_part(s.INTERIOR, stream=main)
+            with torch.cuda.stream(xs):
+                for i, s in enumerate(slabs):
+                    if s.open_below: below2[i].copy_(up2[i - 1], non_blocking=True); s.unpack2(0, below2[i], stream=xs)
+                    if s.open_above: above2[i].copy_(dn2[i + 1], non_blocking=True); s.unpack2(1, above2[i], stream=xs)
+            main.wait_stream(xs)
+            for s in slabs:
+                s.step2_part(s.EDGES, stream=main)
 
     mlups_fused = timed(step_slabs_fused)
     mlups_whole2 = None
@@ -642,6 +657,7 @@ def main():
     ap.add_argument("--sweep-variants", default="0")
     ap.add_argument("--inplace", action="store_true", help="sweep with ONE lattice copy (in-place streaming)")
     ap.add_argument("--slabs", action="store_true", help="N > 1: one lattice cut into z-slabs over the ranks (strong scaling)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="--slabs transport (gloo: ranks may share a GPU)")
     ap.add_argument("--slabs-local", type=int, default=0, help="K z-slabs on this one device (cost of the slab machinery)")
     ap.add_argument("--sweep-sizes", default="", help="e.g. 256x512,4096x8192 (default: all of config 5)")
     args = ap.parse_args()

@@ -102,12 +102,15 @@ int lbm_create(lbm_t **out, int Lx, int Lz, const lbm_params *p);
  *   ... the caller moves the messages (cudaMemcpyAsync between devices, ncclSend/ncclRecv, ...) ...
  *   lbm_slab_unpack(side)    neighbour's message -> my ghost rows of the CURRENT copy
  *   lbm_slab_step(EDGES)     the remaining own rows; then the other copy becomes current.
- * Two steps at once with the two-step kernel (lbm_step2s.cuh), no interior/edge split -- the exchange is a few
- * microseconds beside milliseconds of stepping:
+ * Two steps at once with the two-step kernel (lbm_step2s.cuh):
  *   lbm_slab_pack2(side)     my 6 outermost own rows, all populations, wrap columns included -> message
+ *   lbm_slab_step2_part(INTERIOR)  own rows at least 6 rows from an open side (no ghost row read); overlaps the
+ *                            exchange (Fig. 4); launch it after pack2 in stream order
  *   ... transport ...
  *   lbm_slab_unpack2(side)   neighbour's message -> my 6 ghost rows of the CURRENT copy
- *   lbm_slab_step2           two time steps of the own rows; then the other copy becomes current.
+ *   lbm_slab_step2_part(EDGES)     the 6 own rows next to each open side; then the other copy becomes current.
+ * lbm_slab_step2 = both parts in one launch (after unpack2, no overlap).  A slab too thin for interior rows
+ * (fewer than 6 of them) runs all its rows in EDGES.
  * Results are bit-identical to the whole-lattice run.  Slabs need two lattice copies;
  * lbm_step / lbm_run_host return LBM_ERR_INVALID for them.  lbm_init_rt fills ghost rows too (closed form);
  * after lbm_init_equilibrium / lbm_set_populations the first exchange does. */
@@ -127,6 +130,7 @@ int lbm_slab_step(lbm_t *h, int part, void *stream);
 int lbm_slab_pack2(lbm_t *h, int side, double *msg_dev, void *stream);
 int lbm_slab_unpack2(lbm_t *h, int side, const double *msg_dev, void *stream);
 int lbm_slab_step2(lbm_t *h, void *stream);
+int lbm_slab_step2_part(lbm_t *h, int part, void *stream);
 
 /* Frees the handle and its scratch; never the population buffers. NULL is a no-op. */
 int lbm_destroy(lbm_t *h);

@@ -337,6 +337,12 @@ class Slab(Lattice):
         binding.check(self._lib.lbm_slab_step2(self._h, _stream_ptr(stream, self.device)))
 
     @_on_device
+    def step2_part(self, part: int, stream=None):
+        """The two steps of step2 in two launches groups: INTERIOR (reads no ghost row; after pack2, while the messages
+        travel) and EDGES (after unpack2) -- lbm_slab_step2_part."""
+        binding.check(self._lib.lbm_slab_step2_part(self._h, int(part), _stream_ptr(stream, self.device)))
+
+    @_on_device
     def pack(self, side: int, msg, stream=None):
         binding.check(self._lib.lbm_slab_pack(self._h, int(side), _dptr(msg), _stream_ptr(stream, self.device)))
 

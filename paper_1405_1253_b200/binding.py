@@ -22,7 +22,7 @@ SYMBOLS = [
     "lbm_layout", "lbm_kernel_launches", "lbm_fp64_peak", "lbm_set_variant", "lbm_set_zchunk", "lbm_get_plan", "lbm_tables", "lbm_last_error",
     "lbm_diagnostics", "lbm_rt_scales", "lbm_slab_buffer_bytes", "lbm_create_slab", "lbm_slab_info", "lbm_slab_pack",
     "lbm_slab_unpack", "lbm_slab_step", "lbm_get_window", "lbm_slab_pack2", "lbm_slab_unpack2", "lbm_slab_step2",
-    "lbm_diagnostics_noalloc", "lbm_kinetic_moments",
+    "lbm_diagnostics_noalloc", "lbm_kinetic_moments", "lbm_slab_step2_part",
 ]
 
 
@@ -90,6 +90,7 @@ def load():
     L.lbm_slab_pack2.argtypes = [vp, C.c_int, vp, vp]
     L.lbm_slab_unpack2.argtypes = [vp, C.c_int, vp, vp]
     L.lbm_slab_step2.argtypes = [vp, vp]
+    L.lbm_slab_step2_part.argtypes = [vp, C.c_int, vp]
     L.lbm_slab_pack.argtypes = [vp, C.c_int, vp, vp]
     L.lbm_slab_unpack.argtypes = [vp, C.c_int, vp, vp]
     L.lbm_slab_step.argtypes = [vp, C.c_int, vp]

@@ -141,6 +141,7 @@ struct lbm_handle {
     int zchunk;            // rows per block of the two-step kernel (0 = automatic)
     int sm_count;
     lbm_plan plan;         // cached; invalidated by lbm_set_variant / lbm_set_zchunk
+    lbm_plan plan_interior;   // lbm_slab_step2_part: the plan over the interior rows of a slab
     bool tma_ok;           // tensor maps of both lattice copies encoded (two-step kernel)
     lbm::Step2sMaps maps[2];
     double *scratch;       // device: row diagnostics [8][nz] | results[8] | h_lo[Lx] | h_hi[Lx]
@@ -203,13 +204,11 @@ lbm::StepArgs step_args(const lbm_t *h)
 // wall chunks gather three rows from global memory -- so a launch waits for its slowest block), and takes the
 // one-step kernel where that is predicted to be faster (small lattices).  Constants fitted to the chunk-size runs of
 // profiles/r2_two_step.md section 3.
-const lbm_plan &make_plan(lbm_t *h)
+lbm_plan compute_plan(const lbm_t *h, int rows)
 {
     using S2 = lbm::Step2sWide;
-    if (h->plan.valid) return h->plan;
-    lbm_plan &p = h->plan;
-    p = lbm_plan{};
-    const int Lx = h->Lx, Lz = h->nz, sms = h->sm_count > 0 ? h->sm_count : 148;   // rows to update: a slab's own
+    lbm_plan p = lbm_plan{};
+    const int Lx = h->Lx, Lz = rows, sms = h->sm_count > 0 ? h->sm_count : 148;
     const bool iso_lo = h->wall_kind == 1 && h->wall_lo(), iso_hi = h->wall_kind == 1 && h->wall_hi();
     constexpr int ISO_TRIM = 14;
     const int ns_min = (Lx + S2::TX - 1) / S2::TX;
@@ -257,6 +256,13 @@ const lbm_plan &make_plan(lbm_t *h)
     p.fused = can_fuse && (h->variant == 3 || (h->variant == 0 && t_fused < t_single));
     p.valid = true;
     return p;
+}
+
+// the plan of lbm_step / lbm_slab_step2 over the rows to update (a slab: its own rows), cached
+const lbm_plan &make_plan(lbm_t *h)
+{
+    if (!h->plan.valid) h->plan = compute_plan(h, h->nz);
+    return h->plan;
 }
 
 // periodic images for the two-step kernel's boxes (a1), if copy `i` was last written by anything but that kernel
@@ -331,8 +337,8 @@ void advance(lbm_t *h, int nsteps)
     h->steps += nsteps;
 }
 
-// one launch of the two-step kernel over the rows [zbase, zend) of `a` (lbm_step; lbm_slab_step2)
-int launch_two_step(lbm_t *h, lbm::StepArgs &a, const lbm_plan &plan, cudaStream_t st)
+// one launch of the two-step kernel over the rows [zbase, zend) of `a`, from the current copy into the other one
+int launch_two_step_rows(lbm_t *h, lbm::StepArgs &a, const lbm_plan &plan, cudaStream_t st)
 {
     using S2 = lbm::Step2sWide;
     dim3 grid(plan.strips, plan.chunks);
@@ -353,6 +359,14 @@ int launch_two_step(lbm_t *h, lbm::StepArgs &a, const lbm_plan &plan, cudaStream
     else
         lbm::step2s_kernel<S2, false><<<grid, S2::THREADS, S2::SMEM, st>>>(a, h->maps[h->cur], plan.ZC);
     LAUNCHED(h);
+    return LBM_OK;
+}
+
+// ... over all rows to update, then the other copy is current (lbm_step; lbm_slab_step2)
+int launch_two_step(lbm_t *h, lbm::StepArgs &a, const lbm_plan &plan, cudaStream_t st)
+{
+    int rc = launch_two_step_rows(h, a, plan, st);
+    if (rc) return rc;
     h->wrap_ok[h->cur ^ 1] = a.wrap_store != 0;   // the spare lanes of the seam strips wrote the images (own rows)
     advance(h, 2);                               // a5: swap prv / nxt, once per two steps
     return LBM_OK;
@@ -398,7 +412,7 @@ int create_common(lbm_t **out, int Lx, int rows_stored, const lbm_params *p, con
     h->wrap_ok[0] = h->wrap_ok[1] = false; h->cap_seen = false; h->cap_id = 0;
     h->slab = false; h->Lz_glob = rows_stored; h->z0 = 0; h->nz = rows_stored; h->glo = h->ghi = 0; h->slab_phase = 0;
     h->cur = 0; h->steps = 0; h->launches = 0; h->variant = 0; h->zchunk = 0; h->scratch = nullptr; h->plane_stage = nullptr;
-    h->plan = lbm_plan{};
+    h->plan = lbm_plan{}; h->plan_interior = lbm_plan{};
     h->tma_ok = false;
     h->persist_tb = h->persist_blocks = 0; h->d_counter = nullptr;
     for (auto &s : h->stage) s = nullptr;
@@ -853,6 +867,53 @@ int lbm_slab_step2(lbm_t *h, void *stream)
     return launch_two_step(h, a, plan, (cudaStream_t)stream);
 }
 
+// The same two steps in two parts, so that the exchange of the ghost rows hides behind the bulk (Fig. 4):
+// INTERIOR = own rows at least 6 rows away from an open side (they read no ghost row), EDGES = the 6 rows next to each
+// open side, after lbm_slab_unpack2.  Three launches of the same kernel over disjoint row ranges: bit-identical to
+// lbm_slab_step2.  Slabs too thin to have interior rows run everything in EDGES.
+int lbm_slab_step2_part(lbm_t *h, int part, void *stream)
+{
+    NEED(h);
+    if (!h->slab) return fail(LBM_ERR_INVALID, "lbm_slab_step2_part: not a slab handle");
+    if (h->nz < GHOST_STORED) return fail(LBM_ERR_INVALID, "lbm_slab_step2_part: a slab needs at least %d rows", GHOST_STORED);
+    if (!h->tma_ok) return fail(LBM_ERR_CUDA, "lbm_slab_step2_part: the two-step kernel needs tensor maps (cuTensorMapEncodeTiled failed)");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int own0 = h->glo, own1 = h->glo + h->nz;
+    int i0 = own0 + (h->glo ? GHOST_STORED : 0), i1 = own1 - (h->ghi ? GHOST_STORED : 0);
+    if (i1 - i0 < GHOST_STORED) i0 = i1 = own0;              // no interior worth a launch: EDGES = [own0, own1)
+    lbm::StepArgs a = step_args(h);
+    const lbm_plan &whole = make_plan(h);
+    if (part == LBM_SLAB_INTERIOR) {
+        if (h->slab_phase != 0) return fail(LBM_ERR_INVALID, "lbm_slab_step2_part: a slab step is half done");
+        if (i1 > i0) {
+            if (!h->plan_interior.valid) h->plan_interior = compute_plan(h, i1 - i0);
+            a.zbase = i0; a.zend = i1;
+            int rc = launch_two_step_rows(h, a, h->plan_interior, st);
+            if (rc) return rc;
+        }
+        h->slab_phase = 2;
+        return LBM_OK;
+    }
+    if (part == LBM_SLAB_EDGES) {
+        if (h->slab_phase != 2) return fail(LBM_ERR_INVALID, "lbm_slab_step2_part: launch the interior rows first");
+        lbm_plan edge = whole;                               // same strips; one chunk of the rows of the range
+        edge.trim = 0; edge.chunks = 1;
+        const int ranges[2][2] = {{own0, i1 > i0 ? i0 : own1}, {i1 > i0 ? i1 : own1, own1}};
+        for (auto &r : ranges) {
+            if (r[1] <= r[0]) continue;
+            a.zbase = r[0]; a.zend = r[1];
+            edge.ZC = (r[1] - r[0] + 1) / 2 * 2;
+            int rc = launch_two_step_rows(h, a, edge, st);
+            if (rc) return rc;
+        }
+        h->slab_phase = 0;
+        h->wrap_ok[h->cur ^ 1] = a.wrap_store != 0;
+        advance(h, 2);                                       // a5
+        return LBM_OK;
+    }
+    return fail(LBM_ERR_INVALID, "lbm_slab_step2_part: part must be LBM_SLAB_INTERIOR or LBM_SLAB_EDGES (got %d)", part);
+}
+
 // ---- diagnostics (a6) ------------------------------------------------------------------------------------------------
 int lbm_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T, void *stream)
 {
@@ -1043,7 +1104,7 @@ int lbm_set_zchunk(lbm_t *h, int rows)
     if (rows < 0 || rows == 1 || rows == 2)
         return fail(LBM_ERR_INVALID, "lbm_set_zchunk: rows must be 0 (automatic) or >= 3 (got %d)", rows);
     h->zchunk = rows;
-    h->plan.valid = false;
+    h->plan.valid = false; h->plan_interior.valid = false;
     return LBM_OK;
 }
 
@@ -1052,7 +1113,7 @@ int lbm_set_variant(lbm_t *h, int variant)
     NEED_HOST(h);
     if (variant < 0 || variant > 3) return fail(LBM_ERR_INVALID, "lbm_set_variant: unknown variant %d", variant);
     h->variant = variant;
-    h->plan.valid = false;
+    h->plan.valid = false; h->plan_interior.valid = false;
     return LBM_OK;
 }
 

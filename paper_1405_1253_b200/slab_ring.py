@@ -39,59 +39,90 @@ def exchange_messages(send_up, send_dn, recv_below, recv_above, rank: int, world
 
 class SlabRing:
     """The slab of this rank plus its message buffers.  `step(n)`: pairs of steps with the two-step kernel (6 whole
-    ghost rows per open side and pair, exchanged before the launch: a few microseconds beside milliseconds), an odd
-    last step -- or every step with `fused=False` -- with the one-step kernel: pack on the exchange stream, interior
-    rows on the main stream while the messages travel, unpack, edge rows (interior first)."""
+    ghost rows per open side and pair), an odd last step -- or every step with `fused=False` -- with the one-step
+    kernel (26 population-rows per open side).  Either way the exchange hides behind the bulk (PAPER.md:116-118,
+    Fig. 4): pack on the exchange stream, the interior rows -- which read no ghost row -- on the main stream while the
+    messages travel, unpack, then the edge rows.
+
+    Transport: NCCL moves the device buffers directly.  With any other backend (gloo: the CPU tests, and two ranks
+    sharing one GPU in tests/test_gpu_slab_ring.py) the messages are staged through pinned host buffers; the schedule
+    of kernels and streams is the same."""
 
     def __init__(self, Lx: int, Lz: int, tau: float, g: float, rank: int, world: int, wall_kind: int = 0,
                  T_wall=(1.0, 1.0), device="cuda", group=None):
         import torch
+        import torch.distributed as dist
 
         from . import Slab
         self.rank, self.world, self.group = rank, world, group
         self.z0, self.nz = partition(Lz, world)[rank]
         self.slab = Slab(Lx, Lz, self.z0, self.nz, tau, g, wall_kind=wall_kind, T_wall=T_wall, device=device)
-        self.send_up, self.send_dn, self.recv_below, self.recv_above = (self.slab.new_message() for _ in range(4))
-        self.send2_up, self.send2_dn, self.recv2_below, self.recv2_above = (self.slab.new_message(True) for _ in range(4))
+        # device messages: [send up, send down, received from below, received from above], one-step and two-step sizes
+        self.msg = [self.slab.new_message() for _ in range(4)]
+        self.msg2 = [self.slab.new_message(True) for _ in range(4)]
+        self.staged = world > 1 and dist.get_backend(group) != "nccl"
+        if self.staged:
+            self.host = [torch.empty(m.shape, dtype=m.dtype).pin_memory() for m in self.msg]
+            self.host2 = [torch.empty(m.shape, dtype=m.dtype).pin_memory() for m in self.msg2]
         self.xs = torch.cuda.Stream(device=self.slab.device)
+
+    def _post(self, dev, host):
+        """Starts the transfers of the packed messages `dev[0:2]` (on the exchange stream); returns the requests."""
+        import torch
+        s = self.slab
+        with torch.cuda.stream(self.xs):
+            if not self.staged:
+                return exchange_messages(dev[0], dev[1], dev[2], dev[3], self.rank, self.world, self.group)
+            if s.open_above:
+                host[0].copy_(dev[0], non_blocking=True)
+            if s.open_below:
+                host[1].copy_(dev[1], non_blocking=True)
+        self.xs.synchronize()                                    # the host copies are complete before gloo reads them
+        return exchange_messages(host[0], host[1], host[2], host[3], self.rank, self.world, self.group)
+
+    def _arrived(self, reqs, dev, host):
+        """Waits for the transfers; afterwards the received messages are (or will be, in stream order) in `dev[2:4]`."""
+        import torch
+        s = self.slab
+        with torch.cuda.stream(self.xs):
+            for r in reqs:
+                r.wait()
+            if self.staged:
+                if s.open_below:
+                    dev[2].copy_(host[2], non_blocking=True)
+                if s.open_above:
+                    dev[3].copy_(host[3], non_blocking=True)
 
     def step(self, n: int = 1, fused: bool = True):
         import torch
         s = self.slab
-        main = torch.cuda.current_stream(s.device)
+        main, xs = torch.cuda.current_stream(s.device), self.xs
         pairs = n // 2 if fused else 0
-        for _ in range(pairs):
+        for k in range(n - pairs):                               # `pairs` double steps, then single steps
+            two = k < pairs
+            dev, host = (self.msg2, getattr(self, "host2", None)) if two else (self.msg, getattr(self, "host", None))
+            pack, unpack = (s.pack2, s.unpack2) if two else (s.pack, s.unpack)
+            xs.wait_stream(main)
             if s.open_above:
-                s.pack2(1, self.send2_up, stream=main)
+                pack(1, dev[0], stream=xs)
             if s.open_below:
-                s.pack2(0, self.send2_dn, stream=main)
-            for r in exchange_messages(self.send2_up, self.send2_dn, self.recv2_below, self.recv2_above, self.rank,
-                                       self.world, self.group):
-                r.wait()
+                pack(0, dev[1], stream=xs)
+            if two:
+                main.wait_stream(xs)                             # pack2 refreshes the wrap columns the interior's boxes read
+                s.step2_part(s.INTERIOR, stream=main)            # overlaps the exchange
+            else:
+                s.step_part(s.INTERIOR, stream=main)
+            reqs = self._post(dev, host)
+            self._arrived(reqs, dev, host)
             if s.open_below:
-                s.unpack2(0, self.recv2_below, stream=main)
+                unpack(0, dev[2], stream=xs)
             if s.open_above:
-                s.unpack2(1, self.recv2_above, stream=main)
-            s.step2(stream=main)
-        for _ in range(n - 2 * pairs):
-            self.xs.wait_stream(main)
-            with torch.cuda.stream(self.xs):
-                if s.open_above:
-                    s.pack(1, self.send_up, stream=self.xs)
-                if s.open_below:
-                    s.pack(0, self.send_dn, stream=self.xs)
-                reqs = exchange_messages(self.send_up, self.send_dn, self.recv_below, self.recv_above, self.rank,
-                                         self.world, self.group)
-            s.step_part(s.INTERIOR, stream=main)                 # overlaps the exchange
-            with torch.cuda.stream(self.xs):
-                for r in reqs:
-                    r.wait()
-                if s.open_below:
-                    s.unpack(0, self.recv_below, stream=self.xs)
-                if s.open_above:
-                    s.unpack(1, self.recv_above, stream=self.xs)
-            main.wait_stream(self.xs)
-            s.step_part(s.EDGES, stream=main)
+                unpack(1, dev[3], stream=xs)
+            main.wait_stream(xs)
+            if two:
+                s.step2_part(s.EDGES, stream=main)
+            else:
+                s.step_part(s.EDGES, stream=main)
 
     def close(self):
         self.slab.close()

@@ -179,26 +179,39 @@ def test_slabs_with_exchanged_ghost_rows_equal_the_whole_lattice(pkg, orc, Lx, L
     whole.close()
 
 
-def _run_slabs_fused(pkg, slabs, npairs):
-    """Pairs of steps with the two-step kernel: whole 6-row messages, device-to-device copies, one stream."""
+def _run_slabs_fused(pkg, slabs, npairs, parts=False):
+    """Pairs of steps with the two-step kernel: whole 6-row messages, device-to-device copies.  parts = False: one
+    stream, lbm_slab_step2 after the exchange; parts = True: interior rows on the main stream while the messages are
+    copied and unpacked on a second stream, then the edge rows (lbm_slab_step2_part)."""
     import torch
     up, dn, below, above = ([s.new_message(True) for s in slabs] for _ in range(4))
+    main = torch.cuda.current_stream()
+    xs = torch.cuda.Stream() if parts else main
     for _ in range(npairs):
+        xs.wait_stream(main)
         for i, s in enumerate(slabs):
-            if s.open_above: s.pack2(1, up[i])
-            if s.open_below: s.pack2(0, dn[i])
-        for i, s in enumerate(slabs):
-            if s.open_below: below[i].copy_(up[i - 1], non_blocking=True); s.unpack2(0, below[i])
-            if s.open_above: above[i].copy_(dn[i + 1], non_blocking=True); s.unpack2(1, above[i])
+            if s.open_above: s.pack2(1, up[i], stream=xs)
+            if s.open_below: s.pack2(0, dn[i], stream=xs)
+        if parts:
+            main.wait_stream(xs)
+            for s in slabs:
+                s.step2_part(pkg.Slab.INTERIOR, stream=main)
+        with torch.cuda.stream(xs):
+            for i, s in enumerate(slabs):
+                if s.open_below: below[i].copy_(up[i - 1], non_blocking=True); s.unpack2(0, below[i], stream=xs)
+                if s.open_above: above[i].copy_(dn[i + 1], non_blocking=True); s.unpack2(1, above[i], stream=xs)
+        main.wait_stream(xs)
         for s in slabs:
-            s.step2()
+            if parts: s.step2_part(pkg.Slab.EDGES, stream=main)
+            else: s.step2(stream=main)
     torch.cuda.synchronize()
 
 
+@pytest.mark.parametrize("parts", [False, True])
 @pytest.mark.parametrize("wall_kind", [0, 1])
 @pytest.mark.parametrize("Lx,Lz,cuts,n", [(64, 128, (0, 50, 128), 21), (130, 70, (0, 6, 30, 64, 70), 11), (33, 40, (0, 17, 40), 9),
                                           (600, 300, (0, 100, 207, 300), 14)])
-def test_slabs_with_the_two_step_kernel_equal_the_whole_lattice(pkg, orc, Lx, Lz, cuts, n, wall_kind):
+def test_slabs_with_the_two_step_kernel_equal_the_whole_lattice(pkg, orc, Lx, Lz, cuts, n, wall_kind, parts):
     """z-slabs stepped two steps at a time (lbm_slab_pack2 / unpack2 / step2: 6 whole ghost rows with wrap columns), an
     odd last step with the one-step slab path: bit-identical to the whole lattice, within the oracle tolerance; slabs
     down to 6 rows, several strips, both wall kinds."""
@@ -212,7 +225,7 @@ def test_slabs_with_the_two_step_kernel_equal_the_whole_lattice(pkg, orc, Lx, Lz
     slabs = [pkg.Slab(Lx, Lz, z0, z1 - z0, 0.75, 2e-4, **kw) for z0, z1 in zip(cuts[:-1], cuts[1:])]
     for s in slabs:
         s.set_populations(torch.from_numpy(np.ascontiguousarray(f0[:, s.z0:s.z0 + s.nz])).cuda())
-    _run_slabs_fused(pkg, slabs, n // 2)
+    _run_slabs_fused(pkg, slabs, n // 2, parts=parts)
     _run_slabs(pkg, slabs, n % 2)
     got = torch.cat([s.get_populations() for s in slabs], dim=1)
     assert torch.equal(got, whole.get_populations())
