@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <climits>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -191,6 +192,7 @@ lbm::StepArgs step_args(const lbm_t *h)
     a.wrap_store = 0;
     a.w = 0;
     a.ztrim = 0;
+    a.zsplit = INT_MAX; a.zbase2 = a.zend2 = 0;
     a.zbase = h->glo; a.zend = h->glo + h->nz;
     lbm::fill_offsets(a);
     return a;
@@ -899,12 +901,21 @@ int lbm_slab_step2_part(lbm_t *h, int part, void *stream)
         lbm_plan edge = whole;                               // same strips; one chunk of the rows of the range
         edge.trim = 0; edge.chunks = 1;
         const int ranges[2][2] = {{own0, i1 > i0 ? i0 : own1}, {i1 > i0 ? i1 : own1, own1}};
-        for (auto &r : ranges) {
-            if (r[1] <= r[0]) continue;
-            a.zbase = r[0]; a.zend = r[1];
-            edge.ZC = (r[1] - r[0] + 1) / 2 * 2;
+        if (ranges[0][1] - ranges[0][0] == GHOST_STORED && ranges[1][1] - ranges[1][0] == GHOST_STORED) {
+            // both sides open: the two edge zones as the two chunk rows of ONE launch (twice the blocks, once the time)
+            a.zbase = ranges[0][0]; a.zend = ranges[0][1];
+            a.zsplit = 1; a.zbase2 = ranges[1][0]; a.zend2 = ranges[1][1];
+            edge.ZC = GHOST_STORED; edge.chunks = 2;
             int rc = launch_two_step_rows(h, a, edge, st);
             if (rc) return rc;
+        } else {
+            for (auto &r : ranges) {
+                if (r[1] <= r[0]) continue;
+                a.zbase = r[0]; a.zend = r[1];
+                edge.ZC = (r[1] - r[0] + 1) / 2 * 2;
+                int rc = launch_two_step_rows(h, a, edge, st);
+                if (rc) return rc;
+            }
         }
         h->slab_phase = 0;
         h->wrap_ok[h->cur ^ 1] = a.wrap_store != 0;

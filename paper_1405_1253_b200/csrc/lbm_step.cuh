@@ -37,6 +37,8 @@ struct StepArgs {
     int wrap_store;     // two-step kernel: the consumers of the seam strips maintain the wrap columns (Lx >= 2 XW)
     int w;              // two-step kernel: columns per strip
     int zbase, zend;    // two-step kernel: stored rows [zbase, zend) are updated (a whole lattice: [0, Lz); a z-slab: its own rows)
+    int zsplit, zbase2, zend2;   // two-step kernel: chunk rows blockIdx.y >= zsplit cover a SECOND row range [zbase2, zend2) (the two
+                                 // edge zones of a z-slab in one launch); zsplit = INT_MAX: one range
     int ztrim;          // two-step kernel: chunk c covers rows zbase + [c ZC - ztrim, (c+1) ZC - ztrim) (chunk 0 from 0): wall_kind 1
     // byte offset of population l's pull source relative to the site's own address in plane 0, for sites that
     // need neither wrap nor wall remap: 8 (l plane - e_lz pitch - e_lx).  Host-computed (fill_offsets) so that

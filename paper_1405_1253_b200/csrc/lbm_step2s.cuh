@@ -370,9 +370,11 @@ __global__ void __launch_bounds__(S::THREADS, 1) step2s_kernel(const __grid_cons
     const int w = a.w;                                   // strips of w <= TX columns (w even: TMA boxes start on 16 bytes)
     // a z-slab updates its own rows; its ghost rows are sources only.  ztrim (wall_kind 1): the chunk on an isothermal
     // wall is that many rows shorter, which is what its wall adjustments cost (lbm_api.cu make_plan)
-    const int x0 = blockIdx.x * w, z0 = a.zbase + blockIdx.y * ZC - (blockIdx.y ? a.ztrim : 0);
+    int by = blockIdx.y, zb = a.zbase, ze = a.zend;
+    if (by >= a.zsplit) { by -= a.zsplit; zb = a.zbase2; ze = a.zend2; }   // second row range of the launch (slab edges)
+    const int x0 = blockIdx.x * w, z0 = zb + by * ZC - (by ? a.ztrim : 0);
     const int ncols = min(w, a.Lx - x0);                // output columns of this strip
-    const int zend = min(a.zend, a.zbase + ((int)blockIdx.y + 1) * ZC - a.ztrim);   // output rows [z0, zend)
+    const int zend = min(ze, zb + (by + 1) * ZC - a.ztrim);   // output rows [z0, zend)
     const int rlast = min(a.Lz, zend + 3);              // intermediate rows [max(0, z0-3), rlast)
     const int NP = (zend - z0 + S::R - 1) / S::R;       // consumer passes
     const unsigned bar_full = (unsigned)__cvta_generic_to_shared(&bars[0]);     // [NRB] ring rows written (producers -> consumers)
