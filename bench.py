@@ -36,7 +36,7 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 # until the capture is redone.
 NCU_TRAFFIC = {
     ("rt_single_4096x8192", 1, None, None, "lbm_step.cuh", "f0747db8b6c7e93d7466d3f6ff90472b7d15c26c"): (19.839e9, "profiles/r2_step_kernels_full.md"),
-    ("rt_single_4096x8192", 2, 56, 410, "lbm_step2s.cuh", "c0d3233db4eb1e5fd65842c20e8c94a986c75cb7"): (20.203e9, "profiles/r2_step2s_kernel_full.md"),
+    ("rt_single_4096x8192", 2, 56, 410, "lbm_step2s.cuh", "18b59ca29fdd9930f533092bc42a60318d81d938"): (20.210e9, "profiles/r3_step2s_kernel_full.md"),
 }
 
 

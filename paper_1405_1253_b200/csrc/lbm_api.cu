@@ -950,8 +950,16 @@ int lbm_kinetic_moments(lbm_t *h, double *rho, double *ux, double *uz, double *T
 // one pass over the lattice + one small block; results stay in the handle's scratch
 static int run_diagnostics(lbm_t *h, bool want_rms, double T_d, double T_m, double T_u, cudaStream_t st)
 {
-    if (want_rms) lbm::row_diagnostics_kernel<true><<<h->nz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, h->d_rows());
-    else lbm::row_diagnostics_kernel<false><<<h->nz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, h->d_rows());
+    if (want_rms) {
+        // the row's T and E_k stay in shared memory between the two passes if they fit (Lx <= 12 800), else the row is re-read
+        const size_t smem = sizeof(double) * 2 * (size_t)h->Lx;
+        const int keep = smem <= 200 * 1024;
+        if (keep && smem > 48 * 1024)
+            CUDA_TRY(cudaFuncSetAttribute(lbm::row_diagnostics_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        lbm::row_diagnostics_kernel<true><<<h->nz, lbm::RED_T, keep ? smem : 0, st>>>(h->buf[h->cur], h->layout(), h->g, h->d_rows(), keep);
+    } else {
+        lbm::row_diagnostics_kernel<false><<<h->nz, lbm::RED_T, 0, st>>>(h->buf[h->cur], h->layout(), h->g, h->d_rows(), 0);
+    }
     LAUNCHED(h);
     lbm::final_diagnostics_kernel<<<1, lbm::RED_T, 0, st>>>(h->d_rows(), h->nz, T_d, T_m, T_u, h->d_result());
     LAUNCHED(h);
@@ -1202,7 +1210,7 @@ extern "C" int lbm_diagnostics_noalloc(const void *pop_buf, size_t buf_bytes, in
     // first one, so a correct run never depends on old contents; the part this call uses is zeroed all the same, so that
     // a row kernel that did not run cannot pass the last lattice's numbers off as this one's.
     CUDA_TRY(cudaMemsetAsync(rows, 0, sizeof(double) * 8 * (size_t)Lz, st));
-    lbm::row_diagnostics_kernel<false><<<Lz, lbm::RED_T, 0, st>>>((const double *)pop_buf + lbm::XH, lay, g, rows);
+    lbm::row_diagnostics_kernel<false><<<Lz, lbm::RED_T, 0, st>>>((const double *)pop_buf + lbm::XH, lay, g, rows, 0);
     CUDA_TRY(cudaGetLastError());
     lbm::final_diagnostics_kernel<<<1, lbm::RED_T, 0, st>>>(rows, Lz, T_d, T_m, T_u, result6_dev);
     CUDA_TRY(cudaGetLastError());

@@ -217,10 +217,16 @@ __device__ __forceinline__ double block_sum(double v, double *smem /* RED_T/32 d
 //   out[2][j] = Ekbar(j) = <E_k>_x, E_k = rho |u^(H)|^2/2  (Fig. 9; reading 17)
 //   out[3][j] = Ekrms(j)
 //   out[4..7][j] = row sums of the raw integer-velocity moments sum f, sum e_x f, sum e_z f, sum |e|^2 f
-// WANT_RMS = false skips the second pass over the row (the squared deviations; it re-reads the row from L2).
+// WANT_RMS = false skips the second pass over the row (the squared deviations about the row means).  The second pass
+// needs every site's T and E_k again: with keep != 0 the first pass leaves them in dynamic shared memory (2 Lx doubles;
+// the block is alone on its SM anyway, 226 registers x 256 threads) -- the same values the recomputation gives, so the
+// results are bit-identical -- else it re-reads the row, which comes from DRAM, not L2, on large lattices (ncu:
+// 19.7 GB per launch at 4096x8192 = twice the lattice, profiles/r3_a6_kernels.md).
 template <bool WANT_RMS>
-__global__ void __launch_bounds__(RED_T) row_diagnostics_kernel(const double *__restrict__ src, Layout g, double grav, double *out)
+__global__ void __launch_bounds__(RED_T) row_diagnostics_kernel(const double *__restrict__ src, Layout g, double grav, double *out,
+                                                                int keep)
 {
+    extern __shared__ double rowbuf[];                       // [2][Lx] if WANT_RMS && keep
     __shared__ double sm[RED_T / 32];
     __shared__ double mean[2];
     const int j = blockIdx.x, k = g.k0 + j;
@@ -231,9 +237,12 @@ __global__ void __launch_bounds__(RED_T) row_diagnostics_kernel(const double *__
         const d2q37::RawMoments r = d2q37::raw_moments(f);
         const d2q37::Kinetic m = d2q37::kinetic_from_raw(r);
         const double uz = m.uz + 0.5 * grav;
-        aT += m.T + 0.125 * grav * grav;
-        aE += 0.5 * m.rho * (m.ux * m.ux + uz * uz);
+        const double Ti = m.T + 0.125 * grav * grav, Ei = 0.5 * m.rho * (m.ux * m.ux + uz * uz);
+        aT += Ti;
+        aE += Ei;
         a0 += r.m0; a1 += r.jx; a2 += r.jz; a3 += r.m2;
+        if constexpr (WANT_RMS)
+            if (keep) { rowbuf[i] = Ti; rowbuf[g.Lx + i] = Ei; }
     }
     const double sT = block_sum(aT, sm), sE = block_sum(aE, sm);
     const double s0 = block_sum(a0, sm), s1 = block_sum(a1, sm), s2 = block_sum(a2, sm), s3 = block_sum(a3, sm);
@@ -248,12 +257,18 @@ __global__ void __launch_bounds__(RED_T) row_diagnostics_kernel(const double *__
         const double mT = mean[0], mE = mean[1];
         double vT = 0.0, vE = 0.0;
         for (int i = threadIdx.x; i < g.Lx; i += RED_T) {
-            double f[NPOP];
-            load_site(src, g, i, k, f);
-            const d2q37::Kinetic m = d2q37::kinetic_moments(f);
-            const double uz = m.uz + 0.5 * grav;
-            const double dT = m.T + 0.125 * grav * grav - mT;
-            const double dE = 0.5 * m.rho * (m.ux * m.ux + uz * uz) - mE;
+            double dT, dE;
+            if (keep) {                                      // written by this same thread in the first pass
+                dT = rowbuf[i] - mT;
+                dE = rowbuf[g.Lx + i] - mE;
+            } else {
+                double f[NPOP];
+                load_site(src, g, i, k, f);
+                const d2q37::Kinetic m = d2q37::kinetic_moments(f);
+                const double uz = m.uz + 0.5 * grav;
+                dT = m.T + 0.125 * grav * grav - mT;
+                dE = 0.5 * m.rho * (m.ux * m.ux + uz * uz) - mE;
+            }
             vT += dT * dT;
             vE += dE * dE;
         }

@@ -184,6 +184,14 @@ def test_config4_fullsize_sampled_windows_and_conservation(pkg, orc):
     lu, ld, tbar = lat.mixing_widths(cfg.T_d, cfg.T_m, cfg.T_u)
     assert np.all(np.isfinite(tbar)) and abs(tbar[0] - cfg.T_d) < 1e-3 and abs(tbar[-1] - cfg.T_u) < 1e-3
     assert 2.0 < lu < 12.0 and 2.0 < ld < 12.0 and abs(lu - ld) < 0.5   # tanh front of w = 2.5, diffusing
+    # row profiles at this width (the rows' T and E_k kept in 64 KB of shared memory between the two passes): rows
+    # around the front against the oracle's profiles of the same rows
+    prof = lat.profiles()
+    r0 = cfg.Lz // 2 - 4
+    want = orc.profiles(lat.get_window(r0, 8, 0, cfg.Lx).cpu().numpy(), cfg.g)
+    for a, b, tol in zip(prof, want, (1e-12, 1e-11, 1e-15, 1e-14)):
+        assert np.max(np.abs(a[r0:r0 + 8] - b)) < tol, (np.max(np.abs(a[r0:r0 + 8] - b)), tol)
+    assert want[1].max() > 1e-6
     lat.close()
 
 
